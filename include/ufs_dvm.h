@@ -1,0 +1,139 @@
+/*
+ * ufs_dvm.h -- C ABI of the B200-native DVM step (libufs_dvm.so).
+ *
+ * One explicit time step of the discrete-velocity-method Boltzmann solver of the Unified Flow
+ * Solver's kinetic module (arxiv 1503.00707; citations are lines of the paper text PAPER.md):
+ *
+ *   Eq. 1   df/dt + xi . grad_x f = (1/Kn) I(f,f), non-dimensional, velocity unit sqrt(R T0)
+ *   PAPER.md:93           f lives at the cell centres of a uniform Cartesian velocity grid (nv[0] x nv[1] x nv[2])
+ *                         and of an adaptive octree Cartesian mesh in physical space
+ *   Eq. 2  explicit finite-volume advection; here first-order upwind over every leaf face,
+ *                         2:1 level-jump faces included
+ *   PAPER.md:45           octree rules: levels of direct and of diagonal neighbours differ by at most one
+ *   PAPER.md:51           boundary cells carry the boundary conditions (ghost states)
+ *   PAPER.md:145-163,179  per-cell 5x5 system from the moments of f (here: Newton for the discrete Maxwellian)
+ *   PAPER.md:231          BGK relaxation  -(f - f_eq)/tau
+ *   PAPER.md:81, 207      per-cell kinetic/fluid flag; Maxwellian of the fluid cell at kinetic/fluid faces
+ *
+ * One step, for every KINETIC leaf j and velocity node i (readings in DESIGN.md):
+ *   f*   = f - dt sum_F (A_F/V_j) (xi_i . n_F) f_up          f_up = own value if xi.n > 0, else across F
+ *   rho  = w sum_i (1, xi, |xi|^2) f*                        (fp64 accumulation for either storage type)
+ *   M    = exp(alpha . (1, xi, |xi|^2)),  w sum_i m M = rho  (discrete Maxwellian, Newton)
+ *   f'   = f* + dt nu (M - f*),  nu = nu_prefactor * n * T^(1-visc_exp) / kn
+ *
+ * Conventions.  Every function returns a status code (0 = OK, negative = error); nothing throws,
+ * exits or prints.  "host" / "device" is stated per pointer.  All device work is enqueued on the
+ * CUDA stream given at creation and the calls do not synchronise unless stated; errors of
+ * asynchronous work (including UFS_DVM_ENEWTON) surface at ufs_dvm_sync, ufs_dvm_destroy or, if
+ * already known, at the next call.  The library never allocates f: the two f buffers, the moments
+ * buffer and the stream belong to the caller (PyTorch tensors in the Python binding).
+ */
+#ifndef UFS_DVM_H
+#define UFS_DVM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ufs_dvm_s *ufs_dvm_t; /* opaque handle, owned by the library */
+
+enum { UFS_DVM_OK = 0,
+       UFS_DVM_EINVAL = -1,  /* bad argument, unsupported velocity grid, host-only handle used for device work */
+       UFS_DVM_EMESH = -2,   /* leaves do not tile the cube, overlap, or violate 2:1 balance (faces or diagonals) */
+       UFS_DVM_ECUDA = -3,   /* a CUDA call failed; see ufs_dvm_last_error */
+       UFS_DVM_ENOMEM = -4,
+       UFS_DVM_ENEWTON = -5  /* some cell's Newton solve did not converge (or had n <= 0 or T <= 0) */ };
+enum { UFS_BC_PERIODIC = 0, UFS_BC_SPECULAR = 1, UFS_BC_INFLOW = 2, UFS_BC_OUTFLOW = 3 };
+enum { UFS_CELL_KINETIC = 0, UFS_CELL_FLUID = 1, UFS_CELL_SOLID = 2 }; /* SOLID: removed, specular at its faces */
+enum { UFS_STORE_F64 = 0, UFS_STORE_F32 = 1 };
+/* kinds in the boundary-face list */
+enum { UFS_BF_SPECULAR = 1, UFS_BF_INFLOW = 2, UFS_BF_OUTFLOW = 3, UFS_BF_SOLID = 4, UFS_BF_FLUID = 5 };
+
+/* Problem statement.  All arrays are HOST memory, caller-owned, read during create only. */
+typedef struct {
+    int64_t n_leaves;
+    const uint8_t *level;        /* [n]    octree level of each leaf (edge h = domain_len / 2^level), <= 18 */
+    const uint32_t *ijk;         /* [n][3] integer coordinates of the leaf at its own level                 */
+    const uint8_t *kind;         /* [n]    UFS_CELL_*                                                       */
+    double domain_len;           /* cube edge L                                                             */
+    int32_t bc[6];               /* UFS_BC_* for the sides -x,+x,-y,+y,-z,+z (periodic must be set on both) */
+    double inflow[6][5];         /* (n,ux,uy,uz,T) of the Maxwellian entering through INFLOW sides          */
+    const double *fluid_moments; /* [n][5] (n,ux,uy,uz,T); read for FLUID leaves only; NULL if there are none */
+    int32_t nv[3];               /* velocity nodes per axis; node k: xi = vmin + (k+1/2)(vmax-vmin)/nv      */
+    double vmin[3], vmax[3];
+    double kn;                   /* Knudsen number; +inf switches collisions off                            */
+    double visc_exp;             /* omega in nu ~ T^(1-omega); 0.5 = hard spheres                           */
+    double nu_prefactor;         /* c_nu                                                                     */
+    int32_t storage;             /* UFS_STORE_*: element type of the f buffers                              */
+} ufs_dvm_desc;
+
+/* Flatten the mesh (Morton order, face lists, per-cell upwind gather records, ghost tables), upload it,
+ * and bind the two caller-owned DEVICE buffers f_dev[0], f_dev[1], each n_kinetic * Nv elements of the
+ * storage type, 16-byte aligned, and the CUDA stream (cudaStream_t cast to void*; NULL = default stream).
+ * The buffers are recorded, not read: before the first step the caller fills f_dev[0] with f at t = 0 in
+ * the library's layout, slab s = leaf cell_of_slab[s], slot t = velocity node vel_of_slot[t]
+ * (ufs_dvm_layout).  Validates the tree (EMESH) and the grid (EINVAL: specular sides and SOLID leaves
+ * need vmin = -vmax on the wall-normal axis; Nv * sizeof(element) must fit the on-chip slab buffer). */
+int ufs_dvm_create(const ufs_dvm_desc *desc, void *f_dev[2], void *cuda_stream, ufs_dvm_t *out);
+
+/* Same flattening and validation without touching CUDA: the handle answers ufs_dvm_layout,
+ * ufs_dvm_faces, ufs_dvm_boundary_faces and ufs_dvm_destroy; device calls return EINVAL. */
+int ufs_dvm_create_host(const ufs_dvm_desc *desc, ufs_dvm_t *out);
+
+/* Enqueue nsteps explicit steps of size dt (transport -> moments -> discrete Maxwellian -> BGK
+ * relaxation, one fused kernel per step).  f ping-pongs between the two buffers. */
+int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps);
+
+/* Enqueue the moments of the current f: mom_dev is DEVICE memory, [5][n_kinetic] doubles in slab order:
+ * n, n*ux, n*uy, n*uz, E = (w/2) sum |xi|^2 f  (PAPER.md:237 for the first two). */
+int ufs_dvm_moments(ufs_dvm_t h, double *mom_dev);
+
+/* Wait for the stream and report sticky asynchronous errors (ECUDA, ENEWTON). */
+int ufs_dvm_sync(ufs_dvm_t h);
+
+/* Frees everything the library built (host and device).  The f buffers are not touched. */
+int ufs_dvm_destroy(ufs_dvm_t h);
+
+/* 0 or 1: which of f_dev[] holds the current f. */
+int ufs_dvm_current(ufs_dvm_t h);
+
+/* Layout of the f buffers (HOST outputs, any may be NULL): *n_kinetic; cell_of_slab[n_kinetic] = index into
+ * the caller's leaf list; vel_of_slot[Nv] = canonical velocity index (kz*nv[1] + ky)*nv[0] + kx stored at
+ * each slab slot.  Slabs are in Morton order, slots grouped by velocity octant. */
+int ufs_dvm_layout(ufs_dvm_t h, int64_t *n_kinetic, int64_t *cell_of_slab, int32_t *vel_of_slot);
+
+/* Interior faces between two non-SOLID leaves (HOST outputs; pass NULL arrays to get the count):
+ * owner = leaf on the low side, neigh = leaf on the high side (leaf-list indices), area = min(h)^2,
+ * axis 0/1/2, ratio = level(neigh) - level(owner) in {-1,0,+1}.  Sorted by (Morton rank of owner, axis). */
+int ufs_dvm_faces(ufs_dvm_t h, int64_t *n_faces, int64_t *owner, int64_t *neigh, double *area,
+                  int8_t *axis, int8_t *ratio);
+
+/* Boundary faces of non-SOLID leaves (HOST outputs; NULL arrays for the count): cell (leaf-list index),
+ * axis, side (0 = low, 1 = high), area, kind UFS_BF_*, state = domain side 0..5 for SPECULAR / INFLOW /
+ * OUTFLOW, the SOLID or FLUID leaf's index otherwise. */
+int ufs_dvm_boundary_faces(ufs_dvm_t h, int64_t *n_faces, int64_t *cell, int8_t *axis, int8_t *side,
+                           double *area, int8_t *kind, int64_t *state);
+
+/* End-to-end convenience with HOST buffers (pinned or pageable): copy f_host_in (n_kinetic*Nv elements of
+ * the storage type, library layout) to the current device buffer, run nsteps, compute the moments into
+ * mom_dev_scratch (DEVICE, [5][n_kinetic]) and copy them to mom_host ([5][n_kinetic] doubles); if
+ * f_host_out is not NULL also copy the final f back.  Synchronises the stream before returning. */
+int ufs_dvm_run_host(ufs_dvm_t h, const void *f_host_in, void *f_host_out, double *mom_dev_scratch,
+                     double *mom_host, double dt, int nsteps);
+
+/* Number of kernels this handle has launched so far (step + moments kernels). */
+int64_t ufs_dvm_launch_count(ufs_dvm_t h);
+
+/* Launch geometry of the step kernel: threads per CTA, dynamic shared memory per CTA, vector width in
+ * elements, and 1 if the octant fast path is used (0 = generic per-slot path).  HOST outputs. */
+int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t *threads, int32_t *smem_bytes, int32_t *vec, int32_t *fast);
+
+/* Message of the last error on this handle (valid until the next call on it); never NULL. */
+const char *ufs_dvm_last_error(ufs_dvm_t h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UFS_DVM_H */

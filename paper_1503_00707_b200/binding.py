@@ -1,0 +1,270 @@
+"""Thin Python binding of libufs_dvm.so (include/ufs_dvm.h): same names, argument marshalling only.
+
+Every step of the DVM path runs in the library's CUDA kernels; PyTorch is used here for device
+memory and streams.  There is no CPU fallback: if the library cannot be built or loaded, importing
+this module's functions raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+from .inputs import STORE_F32, Case
+
+OK, EINVAL, EMESH, ECUDA, ENOMEM, ENEWTON = 0, -1, -2, -3, -4, -5
+_CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", ENEWTON: "ENEWTON"}
+
+EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
+           "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
+           "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_last_error"]
+
+
+class ufs_dvm_desc(C.Structure):
+    _fields_ = [("n_leaves", C.c_int64), ("level", C.c_void_p), ("ijk", C.c_void_p), ("kind", C.c_void_p),
+                ("domain_len", C.c_double), ("bc", C.c_int32 * 6), ("inflow", (C.c_double * 5) * 6),
+                ("fluid_moments", C.c_void_p), ("nv", C.c_int32 * 3), ("vmin", C.c_double * 3),
+                ("vmax", C.c_double * 3), ("kn", C.c_double), ("visc_exp", C.c_double),
+                ("nu_prefactor", C.c_double), ("storage", C.c_int32)]
+
+
+class UfsDvmError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"ufs_dvm {_CODES.get(code, code)}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads (building first if stale) the C-ABI library.  Fails loudly; nothing stands in for it."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        vp, i64p = C.c_void_p, C.c_void_p
+        L.ufs_dvm_create.argtypes = [C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p)]
+        L.ufs_dvm_create_host.argtypes = [C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p)]
+        L.ufs_dvm_step.argtypes = [vp, C.c_double, C.c_int]
+        L.ufs_dvm_moments.argtypes = [vp, vp]
+        L.ufs_dvm_sync.argtypes = [vp]
+        L.ufs_dvm_destroy.argtypes = [vp]
+        L.ufs_dvm_current.argtypes = [vp]
+        L.ufs_dvm_layout.argtypes = [vp, C.POINTER(C.c_int64), i64p, vp]
+        L.ufs_dvm_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp]
+        L.ufs_dvm_boundary_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
+        L.ufs_dvm_run_host.argtypes = [vp, vp, vp, vp, vp, C.c_double, C.c_int]
+        L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
+        L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
+        L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def make_desc(case: Case, kn: Optional[float] = None, storage: Optional[int] = None):
+    """ufs_dvm_desc for a Case.  Returns (desc, keepalive list of the host arrays it points to)."""
+    keep = [np.ascontiguousarray(case.level, np.uint8), np.ascontiguousarray(case.ijk, np.uint32),
+            np.ascontiguousarray(case.kind, np.uint8)]
+    d = ufs_dvm_desc()
+    d.n_leaves = case.n_leaves
+    d.level, d.ijk, d.kind = (a.ctypes.data for a in keep)
+    d.domain_len = case.domain_len
+    d.bc[:] = list(case.bc)
+    for s in range(6):
+        d.inflow[s][:] = [float(x) for x in case.inflow[s]]
+    if case.fluid_moments is not None:
+        fm = np.ascontiguousarray(case.fluid_moments, np.float64)
+        keep.append(fm)
+        d.fluid_moments = fm.ctypes.data
+    d.nv[:] = list(case.nv); d.vmin[:] = list(case.vmin); d.vmax[:] = list(case.vmax)
+    d.kn = case.kn if kn is None else kn
+    d.visc_exp, d.nu_prefactor = case.visc_exp, case.nu_prefactor
+    d.storage = case.storage if storage is None else storage
+    return d, keep
+
+
+def _check(h, rc):
+    if rc != OK:
+        msg = lib().ufs_dvm_last_error(h).decode() if h else ""
+        raise UfsDvmError(rc, msg)
+
+
+# ---- the C calls, same names ---------------------------------------------------------------------
+def ufs_dvm_create_host(desc: ufs_dvm_desc) -> C.c_void_p:
+    h = C.c_void_p()
+    rc = lib().ufs_dvm_create_host(C.byref(desc), C.byref(h))
+    if rc != OK:
+        msg = lib().ufs_dvm_last_error(h).decode() if h else ""
+        lib().ufs_dvm_destroy(h)
+        raise UfsDvmError(rc, msg)
+    return h
+
+
+def ufs_dvm_create(desc: ufs_dvm_desc, f_dev_ptrs, cuda_stream: int = 0) -> C.c_void_p:
+    h = C.c_void_p()
+    arr = (C.c_void_p * 2)(f_dev_ptrs[0], f_dev_ptrs[1])
+    rc = lib().ufs_dvm_create(C.byref(desc), arr, C.c_void_p(cuda_stream), C.byref(h))
+    if rc != OK:
+        msg = lib().ufs_dvm_last_error(h).decode() if h else ""
+        lib().ufs_dvm_destroy(h)
+        raise UfsDvmError(rc, msg)
+    return h
+
+
+def ufs_dvm_step(h, dt: float, nsteps: int = 1):
+    _check(h, lib().ufs_dvm_step(h, float(dt), int(nsteps)))
+
+
+def ufs_dvm_moments(h, mom_dev_ptr: int):
+    _check(h, lib().ufs_dvm_moments(h, C.c_void_p(mom_dev_ptr)))
+
+
+def ufs_dvm_sync(h):
+    _check(h, lib().ufs_dvm_sync(h))
+
+
+def ufs_dvm_destroy(h):
+    return lib().ufs_dvm_destroy(h)
+
+
+def ufs_dvm_current(h) -> int:
+    return int(lib().ufs_dvm_current(h))
+
+
+def ufs_dvm_layout(h, Nv: int):
+    """(n_kinetic, cell_of_slab, vel_of_slot); Nv = nv[0]*nv[1]*nv[2] sizes the slot array."""
+    n = C.c_int64()
+    _check(h, lib().ufs_dvm_layout(h, C.byref(n), None, None))
+    cell = np.empty(n.value, np.int64)
+    vel = np.empty(int(Nv), np.int32)
+    _check(h, lib().ufs_dvm_layout(h, C.byref(n), cell.ctypes.data, vel.ctypes.data))
+    return int(n.value), cell, vel
+
+
+def ufs_dvm_faces(h):
+    n = C.c_int64()
+    _check(h, lib().ufs_dvm_faces(h, C.byref(n), None, None, None, None, None))
+    owner = np.empty(n.value, np.int64); neigh = np.empty(n.value, np.int64); area = np.empty(n.value)
+    axis = np.empty(n.value, np.int8); ratio = np.empty(n.value, np.int8)
+    _check(h, lib().ufs_dvm_faces(h, C.byref(n), owner.ctypes.data, neigh.ctypes.data, area.ctypes.data,
+                                  axis.ctypes.data, ratio.ctypes.data))
+    return owner, neigh, area, axis, ratio
+
+
+def ufs_dvm_boundary_faces(h):
+    n = C.c_int64()
+    _check(h, lib().ufs_dvm_boundary_faces(h, C.byref(n), None, None, None, None, None, None))
+    cell = np.empty(n.value, np.int64); axis = np.empty(n.value, np.int8); side = np.empty(n.value, np.int8)
+    area = np.empty(n.value); kind = np.empty(n.value, np.int8); state = np.empty(n.value, np.int64)
+    _check(h, lib().ufs_dvm_boundary_faces(h, C.byref(n), cell.ctypes.data, axis.ctypes.data, side.ctypes.data,
+                                           area.ctypes.data, kind.ctypes.data, state.ctypes.data))
+    return cell, axis, side, area, kind, state
+
+
+def ufs_dvm_run_host(h, f_host_in_ptr: int, f_host_out_ptr: Optional[int], mom_dev_ptr: int, mom_host_ptr: int,
+                     dt: float, nsteps: int):
+    _check(h, lib().ufs_dvm_run_host(h, C.c_void_p(f_host_in_ptr), C.c_void_p(f_host_out_ptr or 0),
+                                     C.c_void_p(mom_dev_ptr), C.c_void_p(mom_host_ptr), float(dt), int(nsteps)))
+
+
+def ufs_dvm_launch_count(h) -> int:
+    return int(lib().ufs_dvm_launch_count(h))
+
+
+def ufs_dvm_kernel_info(h) -> dict:
+    t, s, v, f = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
+    _check(h, lib().ufs_dvm_kernel_info(h, C.byref(t), C.byref(s), C.byref(v), C.byref(f)))
+    return {"threads": t.value, "smem_bytes": s.value, "vec": v.value, "fast": bool(f.value)}
+
+
+def ufs_dvm_last_error(h) -> str:
+    return lib().ufs_dvm_last_error(h).decode()
+
+
+# ---- a small holder: device tensors + handle (memory and streams only) ----------------------------
+class DvmStepper:
+    """Owns the two f tensors and the moments tensor (PyTorch, on `device`) and the library handle.
+
+    f_rows given to / returned by load_canonical / read_canonical are [n_kinetic, Nv] with rows in
+    kinetic-leaf order of the Case and velocities in canonical order; the permutation to and from the
+    library's slab / slot order (ufs_dvm_layout) is applied here, on the host, with numpy."""
+
+    def __init__(self, case: Case, device="cuda:0", kn: Optional[float] = None, storage: Optional[int] = None,
+                 stream=None):
+        import torch
+        self.torch = torch
+        self.case = case
+        self.storage = case.storage if storage is None else storage
+        self.dtype = torch.float32 if self.storage == STORE_F32 else torch.float64
+        self.device = torch.device(device)
+        desc, self._keep = make_desc(case, kn=kn, storage=self.storage)
+        n_kin = int((case.kind == 0).sum())
+        self.Nv = case.Nv
+        with torch.cuda.device(self.device):
+            self.f = [torch.empty((n_kin, self.Nv), dtype=self.dtype, device=self.device) for _ in range(2)]
+            self.mom = torch.empty((5, n_kin), dtype=torch.float64, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.h = ufs_dvm_create(desc, [t.data_ptr() for t in self.f], self.stream.cuda_stream)
+        self.n_kinetic, self.cell_of_slab, self.vel_of_slot = ufs_dvm_layout(self.h, self.Nv)
+        assert self.n_kinetic == n_kin
+        kin = case.kinetic_leaves()
+        row_of_leaf = np.full(case.n_leaves, -1, np.int64)
+        row_of_leaf[kin] = np.arange(kin.size)
+        self.row_of_slab = row_of_leaf[self.cell_of_slab]          # slab -> kinetic row of the Case
+
+    # -- marshalling between canonical host arrays and the device layout
+    def load_canonical(self, f_rows: np.ndarray):
+        torch = self.torch
+        f_rows = np.asarray(f_rows)
+        assert f_rows.shape == (self.n_kinetic, self.Nv)
+        cur = ufs_dvm_current(self.h)
+        chunk = max(1, (1 << 28) // (self.Nv * 8))
+        for s0 in range(0, self.n_kinetic, chunk):
+            rows = self.row_of_slab[s0:s0 + chunk]
+            part = f_rows[rows][:, self.vel_of_slot]
+            self.f[cur][s0:s0 + chunk].copy_(torch.from_numpy(np.ascontiguousarray(part)).to(self.dtype))
+
+    def read_canonical(self, slabs: Optional[np.ndarray] = None) -> np.ndarray:
+        """Current f as float64 [rows, Nv] in canonical order.  With `slabs`, only those slabs, in the
+        order given (rows are then slabs, not Case rows)."""
+        torch = self.torch
+        cur = ufs_dvm_current(self.h)
+        torch.cuda.synchronize(self.device)
+        inv = np.empty(self.Nv, np.int64); inv[self.vel_of_slot] = np.arange(self.Nv)
+        if slabs is not None:
+            idx = torch.as_tensor(np.asarray(slabs, np.int64), device=self.device)
+            return self.f[cur][idx].double().cpu().numpy()[:, inv]
+        out = np.empty((self.n_kinetic, self.Nv))
+        chunk = max(1, (1 << 28) // (self.Nv * 8))
+        for s0 in range(0, self.n_kinetic, chunk):
+            part = self.f[cur][s0:s0 + chunk].double().cpu().numpy()[:, inv]
+            out[self.row_of_slab[s0:s0 + chunk]] = part
+        return out
+
+    def step(self, dt: float, nsteps: int = 1):
+        ufs_dvm_step(self.h, dt, nsteps)
+
+    def moments(self) -> np.ndarray:
+        """[5, n_kinetic] in Case row order: n, n ux, n uy, n uz, E."""
+        ufs_dvm_moments(self.h, self.mom.data_ptr())
+        ufs_dvm_sync(self.h)
+        m = self.mom.cpu().numpy()
+        out = np.empty_like(m)
+        out[:, self.row_of_slab] = m
+        return out
+
+    def sync(self):
+        ufs_dvm_sync(self.h)
+
+    def close(self):
+        if getattr(self, "h", None) is not None:
+            ufs_dvm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,270 @@
+// api.cu -- the C ABI of libufs_dvm.so (include/ufs_dvm.h): handle life cycle, uploads of what the
+// flattener built, and the enqueue calls.  No torch types, no exceptions across the boundary.
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/ufs_dvm.h"
+#include "flatten.hpp"
+#include "kernels.cuh"
+
+using namespace ufs;
+
+struct ufs_dvm_s {
+    FlatMesh mesh;
+    int storage = UFS_STORE_F64;
+    double kn = 0, visc_exp = 0.5, nu_pref = 1, domain_len = 1;
+    bool device = false;
+    void* f[2] = {nullptr, nullptr};
+    int cur = 0;
+    cudaStream_t stream = nullptr;
+    CellRec* d_cells = nullptr;
+    void* d_tables = nullptr;
+    FluidGhost* d_fluid = nullptr;
+    VelDev* d_vel = nullptr;
+    uchar4* d_slot_k = nullptr;
+    int32_t* d_mirror = nullptr;
+    int32_t* d_flags = nullptr;
+    StepLaunch plan{};
+    int64_t launches = 0;
+    int sticky = UFS_DVM_OK;
+    std::string err;
+};
+
+namespace {
+
+int fail(ufs_dvm_t h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+int cuda_fail(ufs_dvm_t h, cudaError_t e, const char* what) {
+    h->sticky = UFS_DVM_ECUDA;
+    return fail(h, UFS_DVM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call, what)                                        \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(h, e__, what); \
+    } while (0)
+
+template <typename T>
+int upload(ufs_dvm_t h, T** dst, const void* src, size_t bytes, const char* what) {
+    *dst = nullptr;
+    if (bytes == 0) return UFS_DVM_OK;
+    CU(cudaMalloc(reinterpret_cast<void**>(dst), bytes), what);
+    CU(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, h->stream), what);
+    return UFS_DVM_OK;
+}
+
+StepParams make_params(ufs_dvm_t h, double dt) {
+    StepParams p{};
+    const VelLayout& v = h->mesh.vel;
+    p.f_in = h->f[h->cur];
+    p.f_out = h->f[h->cur ^ 1];
+    p.cells = h->d_cells;
+    p.tables = h->d_tables;
+    p.fluid = h->d_fluid;
+    p.vel = h->d_vel;
+    p.slot_k = h->d_slot_k;
+    p.mirror_slot = h->d_mirror;
+    p.flags = h->d_flags;
+    p.Nv = v.Nv;
+    p.n_kin = (int32_t)h->mesh.n_kin;
+    for (int a = 0; a < 3; a++) { p.nv[a] = v.nv[a]; p.nh[a] = v.nh[a]; }
+    p.collide = std::isinf(h->kn) ? 0 : 1;
+    p.dt = dt;
+    p.w = v.w;
+    p.inv_len = 1.0 / h->domain_len;
+    p.inv_kn = p.collide ? 1.0 / h->kn : 0.0;
+    p.visc_exp = h->visc_exp;
+    p.nu_pref = h->nu_pref;
+    return p;
+}
+
+int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out) {
+    if (!out) return UFS_DVM_EINVAL;
+    *out = nullptr;
+    if (!desc) return UFS_DVM_EINVAL;
+    ufs_dvm_t h = new (std::nothrow) ufs_dvm_s();
+    if (!h) return UFS_DVM_ENOMEM;
+    *out = h;  // returned even on failure so that the caller can read last_error, then destroy
+    h->storage = desc->storage;
+    h->kn = desc->kn; h->visc_exp = desc->visc_exp; h->nu_pref = desc->nu_prefactor; h->domain_len = desc->domain_len;
+    try {
+        std::string err;
+        int rc = flatten(*desc, h->mesh, err);
+        if (rc) return fail(h, rc, err);
+    } catch (const std::bad_alloc&) {
+        return fail(h, UFS_DVM_ENOMEM, "out of host memory while flattening");
+    } catch (...) {
+        return fail(h, UFS_DVM_EINVAL, "unexpected failure while flattening");
+    }
+    const char* why = "";
+    int rc = step_plan(h->storage, h->mesh.vel, &h->plan, &why);
+    if (rc) return fail(h, rc, why);
+    return UFS_DVM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ufs_dvm_create_host(const ufs_dvm_desc* desc, ufs_dvm_t* out) { return create_common(desc, out); }
+
+int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, ufs_dvm_t* out) {
+    int rc = create_common(desc, out);
+    if (rc) return rc;
+    ufs_dvm_t h = *out;
+    if (!f_dev || ((!f_dev[0] || !f_dev[1]) && h->mesh.n_kin > 0)) return fail(h, UFS_DVM_EINVAL, "f_dev[0] and f_dev[1] must be device buffers");
+    if (h->mesh.n_kin > 0 && (f_dev[0] == f_dev[1] || ((uintptr_t)f_dev[0] & 15) || ((uintptr_t)f_dev[1] & 15)))
+        return fail(h, UFS_DVM_EINVAL, "the two f buffers must be distinct and 16-byte aligned");
+    h->f[0] = f_dev[0]; h->f[1] = f_dev[1];
+    h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    h->device = true;
+    const FlatMesh& m = h->mesh;
+    const VelLayout& v = m.vel;
+    if ((rc = upload(h, &h->d_cells, m.recs.data(), m.recs.size() * sizeof(CellRec), "upload cell records"))) return rc;
+    if ((rc = upload(h, &h->d_fluid, m.fluid.data(), m.fluid.size() * sizeof(FluidGhost), "upload fluid ghosts"))) return rc;
+    VelDev vd{};
+    std::memcpy(vd.xi, v.xi, sizeof vd.xi);
+    for (int a = 0; a < 3; a++) { vd.nv[a] = v.nv[a]; vd.nh[a] = v.nh[a]; }
+    if ((rc = upload(h, &h->d_vel, &vd, sizeof vd, "upload velocity grid"))) return rc;
+    if ((rc = upload(h, &h->d_slot_k, v.slot_k.data(), v.slot_k.size(), "upload slot table"))) return rc;
+    std::vector<int32_t> mir((size_t)3 * v.Nv);
+    for (int a = 0; a < 3; a++) std::memcpy(mir.data() + (size_t)a * v.Nv, v.mirror_slot[a].data(), (size_t)v.Nv * 4);
+    if ((rc = upload(h, &h->d_mirror, mir.data(), mir.size() * 4, "upload mirror table"))) return rc;
+    // inflow ghost tables in the storage type
+    std::vector<float> tab32;
+    const void* tab = m.tables.data();
+    size_t tab_bytes = m.tables.size() * 8;
+    if (h->storage == UFS_STORE_F32) {
+        tab32.assign(m.tables.begin(), m.tables.end());
+        tab = tab32.data();
+        tab_bytes = tab32.size() * 4;
+    }
+    if ((rc = upload(h, &h->d_tables, tab, tab_bytes, "upload inflow tables"))) return rc;
+    CU(cudaMalloc(reinterpret_cast<void**>(&h->d_flags), 4), "allocate flags");
+    CU(cudaMemsetAsync(h->d_flags, 0, 4, h->stream), "clear flags");
+    CU(cudaStreamSynchronize(h->stream), "upload");  // the host vectors above die at return
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (!(dt > 0) || nsteps < 0) return fail(h, UFS_DVM_EINVAL, "dt must be positive and nsteps >= 0");
+    for (int s = 0; s < nsteps; s++) {
+        const StepParams p = make_params(h, dt);
+        CU(launch_step(h->storage, h->plan, p, h->stream), "step kernel launch");
+        h->cur ^= 1;
+        if (h->mesh.n_kin > 0) h->launches++;
+    }
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_moments(ufs_dvm_t h, double* mom_dev) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (!mom_dev && h->mesh.n_kin > 0) return fail(h, UFS_DVM_EINVAL, "mom_dev is NULL");
+    const StepParams p = make_params(h, 1.0);
+    CU(launch_moments(h->storage, p, h->f[h->cur], mom_dev, h->stream), "moments kernel launch");
+    if (h->mesh.n_kin > 0) h->launches++;
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_sync(ufs_dvm_t h) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    CU(cudaStreamSynchronize(h->stream), "stream synchronize");
+    int32_t flags = 0;
+    CU(cudaMemcpy(&flags, h->d_flags, 4, cudaMemcpyDeviceToHost), "read flags");
+    if ((flags & 1) && h->sticky == UFS_DVM_OK) {
+        h->sticky = UFS_DVM_ENEWTON;
+        h->err = "Newton iteration for the discrete Maxwellian failed in at least one cell (n <= 0, T <= 0 or no convergence)";
+    }
+    return h->sticky;
+}
+
+int ufs_dvm_destroy(ufs_dvm_t h) {
+    if (!h) return UFS_DVM_OK;
+    int rc = UFS_DVM_OK;
+    if (h->device) {
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess) rc = UFS_DVM_ECUDA;
+        cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
+        cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags);
+    }
+    delete h;
+    return rc;
+}
+
+int ufs_dvm_current(ufs_dvm_t h) { return h ? h->cur : UFS_DVM_EINVAL; }
+
+int ufs_dvm_layout(ufs_dvm_t h, int64_t* n_kinetic, int64_t* cell_of_slab, int32_t* vel_of_slot) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (n_kinetic) *n_kinetic = h->mesh.n_kin;
+    if (cell_of_slab) std::memcpy(cell_of_slab, h->mesh.cell_of_slab.data(), (size_t)h->mesh.n_kin * 8);
+    if (vel_of_slot) std::memcpy(vel_of_slot, h->mesh.vel.vel_of_slot.data(), (size_t)h->mesh.vel.Nv * 4);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_faces(ufs_dvm_t h, int64_t* n_faces, int64_t* owner, int64_t* neigh, double* area, int8_t* axis, int8_t* ratio) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    const size_t n = m.f_owner.size();
+    if (n_faces) *n_faces = (int64_t)n;
+    if (owner) std::memcpy(owner, m.f_owner.data(), n * 8);
+    if (neigh) std::memcpy(neigh, m.f_neigh.data(), n * 8);
+    if (area) std::memcpy(area, m.f_area.data(), n * 8);
+    if (axis) std::memcpy(axis, m.f_axis.data(), n);
+    if (ratio) std::memcpy(ratio, m.f_ratio.data(), n);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_boundary_faces(ufs_dvm_t h, int64_t* n_faces, int64_t* cell, int8_t* axis, int8_t* side, double* area,
+                           int8_t* kind, int64_t* state) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    const size_t n = m.b_cell.size();
+    if (n_faces) *n_faces = (int64_t)n;
+    if (cell) std::memcpy(cell, m.b_cell.data(), n * 8);
+    if (axis) std::memcpy(axis, m.b_axis.data(), n);
+    if (side) std::memcpy(side, m.b_side.data(), n);
+    if (area) std::memcpy(area, m.b_area.data(), n * 8);
+    if (kind) std::memcpy(kind, m.b_kind.data(), n);
+    if (state) std::memcpy(state, m.b_state.data(), n * 8);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, double* mom_dev_scratch, double* mom_host,
+                     double dt, int nsteps) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (!f_host_in || !mom_dev_scratch || !mom_host) return fail(h, UFS_DVM_EINVAL, "NULL buffer");
+    const size_t bytes = (size_t)h->mesh.n_kin * (size_t)h->mesh.vel.Nv * (h->storage == UFS_STORE_F32 ? 4 : 8);
+    CU(cudaMemcpyAsync(h->f[h->cur], f_host_in, bytes, cudaMemcpyHostToDevice, h->stream), "copy f to the device");
+    int rc = ufs_dvm_step(h, dt, nsteps);
+    if (rc) return rc;
+    if ((rc = ufs_dvm_moments(h, mom_dev_scratch))) return rc;
+    CU(cudaMemcpyAsync(mom_host, mom_dev_scratch, (size_t)h->mesh.n_kin * 40, cudaMemcpyDeviceToHost, h->stream), "copy moments to the host");
+    if (f_host_out) CU(cudaMemcpyAsync(f_host_out, h->f[h->cur], bytes, cudaMemcpyDeviceToHost, h->stream), "copy f to the host");
+    return ufs_dvm_sync(h);
+}
+
+int64_t ufs_dvm_launch_count(ufs_dvm_t h) { return h ? h->launches : 0; }
+
+int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int32_t* vec, int32_t* fast) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (threads) *threads = h->plan.threads;
+    if (smem_bytes) *smem_bytes = h->plan.smem_bytes;
+    if (vec) *vec = h->plan.vec;
+    if (fast) *fast = h->plan.fast;
+    return UFS_DVM_OK;
+}
+
+const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }
+
+}  // extern "C"

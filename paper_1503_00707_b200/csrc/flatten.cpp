@@ -1,0 +1,378 @@
+// flatten.cpp -- host-side octree flattener (see flatten.hpp).  Neighbour search by binary search in
+// the Morton-sorted leaf array: a leaf at level l covers the key interval [key, key + 8^(lmax-l)), the
+// leaves tile [0, 8^lmax), so "which leaf covers this point" is one upper_bound.
+#include "flatten.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+namespace ufs {
+namespace {
+
+inline uint64_t spread3(uint64_t v) {  // 21 bits -> every third bit
+    v &= 0x1fffffULL;
+    v = (v | (v << 32)) & 0x1f00000000ffffULL;
+    v = (v | (v << 16)) & 0x1f0000ff0000ffULL;
+    v = (v | (v << 8)) & 0x100f00f00f00f00fULL;
+    v = (v | (v << 4)) & 0x10c30c30c30c30c3ULL;
+    v = (v | (v << 2)) & 0x1249249249249249ULL;
+    return v;
+}
+// depth-first order with child index x + 2y + 4z
+inline uint64_t morton(uint64_t x, uint64_t y, uint64_t z) { return spread3(x) | (spread3(y) << 1) | (spread3(z) << 2); }
+
+struct Tree {
+    const ufs_dvm_desc& d;
+    int lmax;
+    std::vector<uint64_t> start;  // Morton-sorted start keys
+    std::vector<int64_t> order;   // rank -> leaf
+    // leaf covering the finest-level point (x,y,z)
+    int64_t cover(int64_t x, int64_t y, int64_t z) const {
+        uint64_t key = morton((uint64_t)x, (uint64_t)y, (uint64_t)z);
+        auto it = std::upper_bound(start.begin(), start.end(), key);
+        return order[(it - start.begin()) - 1];
+    }
+};
+
+enum : int8_t { NB_NONE = 0, NB_LEAF = 1, NB_DOMAIN = 2 };
+struct Nb {
+    int8_t type[4];
+    int8_t cnt;
+    int64_t id[4];  // leaf, or domain side
+};
+
+int build_velocity(const ufs_dvm_desc& d, VelLayout& v, std::string& err) {
+    v.Nv = 1;
+    v.w = 1.0;
+    v.fast = true;
+    for (int a = 0; a < 3; a++) {
+        if (d.nv[a] < 1 || d.nv[a] > NV_MAX) { err = "nv must be in 1.." + std::to_string(NV_MAX) + " on every axis"; return UFS_DVM_EINVAL; }
+        if (!(d.vmax[a] > d.vmin[a])) { err = "vmax must exceed vmin"; return UFS_DVM_EINVAL; }
+        v.nv[a] = d.nv[a];
+        v.Nv *= d.nv[a];
+        const double dv = (d.vmax[a] - d.vmin[a]) / d.nv[a];
+        v.w *= dv;
+        v.ncls[a][0] = v.ncls[a][1] = v.ncls[a][2] = 0;
+        for (int k = 0; k < d.nv[a]; k++) v.xi[a][k] = d.vmin[a] + (k + 0.5) * dv;
+        v.symmetric[a] = std::fabs(d.vmin[a] + d.vmax[a]) <= 1e-14 * std::fabs(d.vmax[a]);
+        if (v.symmetric[a]) {  // make the nodes exactly mirror-symmetric so |xi| depends on the rank only
+            for (int k = 0; k < d.nv[a] / 2; k++) v.xi[a][k] = -v.xi[a][d.nv[a] - 1 - k];
+            if (d.nv[a] % 2) v.xi[a][d.nv[a] / 2] = 0.0;
+        }
+        for (int k = 0; k < d.nv[a]; k++) v.ncls[a][v.xi[a][k] < 0 ? 0 : (v.xi[a][k] > 0 ? 1 : 2)]++;
+        v.nh[a] = d.nv[a] / 2;
+        if (!(v.symmetric[a] && d.nv[a] % 2 == 0)) v.fast = false;
+        if (v.ncls[a][2] > 1) { err = "internal: two zero nodes"; return UFS_DVM_EINVAL; }
+    }
+    // class and rank (by increasing |xi|) of every node
+    int cls[3][NV_MAX], rk[3][NV_MAX];
+    for (int a = 0; a < 3; a++)
+        for (int k = 0; k < v.nv[a]; k++) {
+            const double x = v.xi[a][k];
+            if (x < 0) { cls[a][k] = 0; rk[a][k] = v.ncls[a][0] - 1 - k; }       // negative nodes come first
+            else if (x > 0) { cls[a][k] = 1; rk[a][k] = k - (v.nv[a] - v.ncls[a][1]); }
+            else { cls[a][k] = 2; rk[a][k] = 0; }
+        }
+    // groups in order (cz, cy, cx), cx fastest; with no zero class this is octant sx + 2 sy + 4 sz
+    int64_t gstart[3][3][3];
+    int64_t off = 0;
+    for (int cz = 0; cz < 3; cz++) for (int cy = 0; cy < 3; cy++) for (int cx = 0; cx < 3; cx++) {
+        gstart[cz][cy][cx] = off;
+        off += (int64_t)v.ncls[0][cx] * v.ncls[1][cy] * v.ncls[2][cz];
+    }
+    v.vel_of_slot.assign(v.Nv, -1);
+    v.slot_of_vel.assign(v.Nv, -1);
+    v.slot_k.assign(v.Nv * 4, 0);
+    for (int kz = 0; kz < v.nv[2]; kz++) for (int ky = 0; ky < v.nv[1]; ky++) for (int kx = 0; kx < v.nv[0]; kx++) {
+        const int cx = cls[0][kx], cy = cls[1][ky], cz = cls[2][kz];
+        const int64_t slot = gstart[cz][cy][cx] + ((int64_t)rk[2][kz] * v.ncls[1][cy] + rk[1][ky]) * v.ncls[0][cx] + rk[0][kx];
+        const int64_t can = ((int64_t)kz * v.nv[1] + ky) * v.nv[0] + kx;
+        v.vel_of_slot[slot] = (int32_t)can;
+        v.slot_of_vel[can] = (int32_t)slot;
+        v.slot_k[slot * 4 + 0] = (uint8_t)kx; v.slot_k[slot * 4 + 1] = (uint8_t)ky; v.slot_k[slot * 4 + 2] = (uint8_t)kz;
+    }
+    for (int a = 0; a < 3; a++) {
+        v.mirror_slot[a].assign(v.Nv, -1);
+        if (!v.symmetric[a]) continue;
+        for (int64_t s = 0; s < v.Nv; s++) {
+            int k[3] = {v.slot_k[s * 4], v.slot_k[s * 4 + 1], v.slot_k[s * 4 + 2]};
+            k[a] = v.nv[a] - 1 - k[a];
+            v.mirror_slot[a][s] = v.slot_of_vel[((int64_t)k[2] * v.nv[1] + k[1]) * v.nv[0] + k[0]];
+        }
+    }
+    return UFS_DVM_OK;
+}
+
+// pointwise Maxwellian n/(2 pi T)^{3/2} exp(-|xi-u|^2/2T) as separable factors (reading G13)
+void maxwell_factors(const double* prim, const VelLayout& v, FluidGhost& g) {
+    const double PI = 3.14159265358979323846;
+    const double n = prim[0], T = prim[4];
+    g.amp = n / std::pow(2.0 * PI * T, 1.5);
+    for (int a = 0; a < 3; a++)
+        for (int k = 0; k < v.nv[a]; k++) {
+            const double c = v.xi[a][k] - prim[1 + a];
+            g.g[a][k] = std::exp(-c * c / (2.0 * T));
+        }
+}
+
+}  // namespace
+
+int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
+    if (d.n_leaves <= 0 || !d.level || !d.ijk || !d.kind) { err = "empty or NULL leaf list"; return UFS_DVM_EINVAL; }
+    if (!(d.domain_len > 0)) { err = "domain_len must be positive"; return UFS_DVM_EINVAL; }
+    if (d.storage != UFS_STORE_F64 && d.storage != UFS_STORE_F32) { err = "unknown storage type"; return UFS_DVM_EINVAL; }
+    if (!(d.kn > 0)) { err = "kn must be positive (+inf = collisions off)"; return UFS_DVM_EINVAL; }
+    for (int a = 0; a < 3; a++) {
+        for (int s = 0; s < 2; s++)
+            if (d.bc[2 * a + s] < UFS_BC_PERIODIC || d.bc[2 * a + s] > UFS_BC_OUTFLOW) { err = "unknown boundary code"; return UFS_DVM_EINVAL; }
+        if ((d.bc[2 * a] == UFS_BC_PERIODIC) != (d.bc[2 * a + 1] == UFS_BC_PERIODIC)) { err = "periodic must be set on both sides of an axis"; return UFS_DVM_EINVAL; }
+    }
+    int rc = build_velocity(d, m.vel, err);
+    if (rc) return rc;
+    const VelLayout& vel = m.vel;
+    const int64_t n = d.n_leaves;
+    m.n_leaves = n;
+
+    // ---- Morton order and the tiling check --------------------------------------------------------
+    int lmax = 0;
+    bool any_solid = false, any_fluid = false;
+    for (int64_t j = 0; j < n; j++) {
+        if (d.level[j] > 18) { err = "level > 18"; return UFS_DVM_EINVAL; }
+        if (d.kind[j] > UFS_CELL_SOLID) { err = "unknown cell kind"; return UFS_DVM_EINVAL; }
+        lmax = std::max<int>(lmax, d.level[j]);
+        any_solid |= d.kind[j] == UFS_CELL_SOLID;
+        any_fluid |= d.kind[j] == UFS_CELL_FLUID;
+    }
+    if (any_fluid && !d.fluid_moments) { err = "FLUID leaves need fluid_moments"; return UFS_DVM_EINVAL; }
+    m.lmax = lmax;
+    std::vector<uint64_t> key(n);
+    for (int64_t j = 0; j < n; j++) {
+        const int l = d.level[j];
+        const uint32_t nl = 1u << l;
+        const uint32_t* c = d.ijk + 3 * j;
+        if (c[0] >= nl || c[1] >= nl || c[2] >= nl) { err = "leaf " + std::to_string(j) + " lies outside the cube"; return UFS_DVM_EMESH; }
+        const int sh = lmax - l;
+        key[j] = morton((uint64_t)c[0] << sh, (uint64_t)c[1] << sh, (uint64_t)c[2] << sh);
+    }
+    m.order.resize(n);
+    std::iota(m.order.begin(), m.order.end(), (int64_t)0);
+    std::sort(m.order.begin(), m.order.end(), [&](int64_t a, int64_t b) { return key[a] != key[b] ? key[a] < key[b] : d.level[a] < d.level[b]; });
+    Tree t{d, lmax, {}, m.order};
+    t.start.resize(n);
+    uint64_t expect = 0;
+    for (int64_t r = 0; r < n; r++) {
+        const int64_t j = m.order[r];
+        t.start[r] = key[j];
+        if (key[j] != expect) {
+            err = std::string(key[j] < expect ? "leaves overlap" : "leaves leave a gap") + " at leaf " + std::to_string(j);
+            return UFS_DVM_EMESH;
+        }
+        expect = key[j] + (1ULL << (3 * (lmax - d.level[j])));
+    }
+    if (expect != (1ULL << (3 * lmax))) { err = "leaves do not fill the cube"; return UFS_DVM_EMESH; }
+    m.rank.resize(n);
+    for (int64_t r = 0; r < n; r++) m.rank[m.order[r]] = r;
+
+    // ---- neighbour search (6 faces) and the 26-neighbour 2:1 check --------------------
+    std::vector<Nb> nb((size_t)n * 6);
+    int bad = 0;
+    const int64_t NF = (int64_t)1 << lmax;
+#pragma omp parallel for schedule(static) reduction(| : bad)
+    for (int64_t j = 0; j < n; j++) {
+        const int l = d.level[j];
+        const int sh = lmax - l;
+        const int64_t nl = (int64_t)1 << l;
+        const int64_t c[3] = {d.ijk[3 * j], d.ijk[3 * j + 1], d.ijk[3 * j + 2]};
+        // 26 neighbours: the covering leaf of the adjacent same-size block may not be coarser than l-1
+        for (int dz = -1; dz <= 1; dz++) for (int dy = -1; dy <= 1; dy++) for (int dx = -1; dx <= 1; dx++) {
+            if (!dx && !dy && !dz) continue;
+            int64_t q[3] = {c[0] + dx, c[1] + dy, c[2] + dz};
+            bool outside = false;
+            for (int a = 0; a < 3; a++) {
+                if (q[a] < 0 || q[a] >= nl) {
+                    if (d.bc[2 * a] == UFS_BC_PERIODIC) q[a] = (q[a] + nl) % nl;
+                    else outside = true;
+                }
+            }
+            if (outside) continue;
+            const int64_t cov = t.cover(q[0] << sh, q[1] << sh, q[2] << sh);
+            if ((int)d.level[cov] < l - 1) bad |= 1;
+        }
+        for (int dir = 0; dir < 6; dir++) {
+            Nb& e = nb[(size_t)j * 6 + dir];
+            std::memset(&e, 0, sizeof e);
+            const int a = dir >> 1, s = (dir & 1) ? 1 : -1;
+            int64_t q[3] = {c[0], c[1], c[2]};
+            q[a] += s;
+            if (q[a] < 0 || q[a] >= nl) {
+                if (d.bc[dir] == UFS_BC_PERIODIC) q[a] = (q[a] + nl) % nl;
+                else { e.cnt = 1; e.type[0] = NB_DOMAIN; e.id[0] = dir; continue; }
+            }
+            const int64_t cov = t.cover(q[0] << sh, q[1] << sh, q[2] << sh);
+            const int lc = d.level[cov];
+            if (lc <= l) {  // same level or coarser: one face
+                if (lc < l - 1) bad |= 1;
+                e.cnt = 1; e.type[0] = NB_LEAF; e.id[0] = cov;
+                continue;
+            }
+            // finer: the four level-(l+1) children of the adjacent block that touch the shared face
+            if (sh < 1) { bad |= 1; continue; }
+            const int b1 = (a + 1) % 3, b2 = (a + 2) % 3;
+            int cnt = 0;
+            for (int u = 0; u < 2; u++) for (int w = 0; w < 2; w++) {
+                int64_t cc[3];
+                cc[a] = 2 * q[a] + (s > 0 ? 0 : 1);
+                cc[b1] = 2 * q[b1] + u;
+                cc[b2] = 2 * q[b2] + w;
+                const int64_t ch = t.cover(cc[0] << (sh - 1), cc[1] << (sh - 1), cc[2] << (sh - 1));
+                if ((int)d.level[ch] != l + 1) bad |= 1;
+                e.type[cnt] = NB_LEAF; e.id[cnt] = ch; cnt++;
+            }
+            e.cnt = 4;
+        }
+    }
+    (void)NF;
+    if (bad) { err = "octree is not 2:1 balanced (face, edge or corner neighbours differ by more than one level)"; return UFS_DVM_EMESH; }
+
+    // ---- specular reflection needs a mirror-symmetric velocity grid on the wall-normal axis -----------
+    for (int a = 0; a < 3; a++) {
+        const bool need = any_solid || d.bc[2 * a] == UFS_BC_SPECULAR || d.bc[2 * a + 1] == UFS_BC_SPECULAR;
+        if (need && !vel.symmetric[a]) { err = "specular walls / SOLID leaves need vmin = -vmax on axis " + std::to_string(a); return UFS_DVM_EINVAL; }
+    }
+
+    // ---- slabs: kinetic leaves in Morton order -----------------------------------------------------
+    m.slab_of_leaf.assign(n, -1);
+    m.cell_of_slab.clear();
+    for (int64_t r = 0; r < n; r++) {
+        const int64_t j = m.order[r];
+        if (d.kind[j] == UFS_CELL_KINETIC) { m.slab_of_leaf[j] = (int64_t)m.cell_of_slab.size(); m.cell_of_slab.push_back(j); }
+    }
+    m.n_kin = (int64_t)m.cell_of_slab.size();
+    if (m.n_kin >= (1 << SRC_SHIFT)) { err = "too many kinetic leaves for the 28-bit source index"; return UFS_DVM_EINVAL; }
+
+    // ---- face lists, in Morton order of the owner ----------------------------------------------------
+    for (int64_t r = 0; r < n; r++) {
+        const int64_t j = m.order[r];
+        if (d.kind[j] == UFS_CELL_SOLID) continue;
+        const double h = d.domain_len / (double)((int64_t)1 << d.level[j]);
+        for (int a = 0; a < 3; a++) {
+            for (int side = 0; side < 2; side++) {
+                const Nb& e = nb[(size_t)j * 6 + 2 * a + side];
+                for (int k = 0; k < e.cnt; k++) {
+                    const double area = (e.cnt == 4) ? 0.25 * h * h : h * h;  // min(h_o,h_n)^2: our own face is never the larger one unless cnt==4
+                    if (e.type[k] == NB_DOMAIN) {
+                        const int bc = d.bc[e.id[k]];
+                        m.b_cell.push_back(j); m.b_axis.push_back((int8_t)a); m.b_side.push_back((int8_t)side); m.b_area.push_back(area);
+                        m.b_kind.push_back((int8_t)(bc == UFS_BC_SPECULAR ? UFS_BF_SPECULAR : bc == UFS_BC_INFLOW ? UFS_BF_INFLOW : UFS_BF_OUTFLOW));
+                        m.b_state.push_back(e.id[k]);
+                        continue;
+                    }
+                    const int64_t q = e.id[k];
+                    if (d.kind[q] == UFS_CELL_SOLID) {
+                        m.b_cell.push_back(j); m.b_axis.push_back((int8_t)a); m.b_side.push_back((int8_t)side); m.b_area.push_back(area);
+                        m.b_kind.push_back((int8_t)UFS_BF_SOLID); m.b_state.push_back(q);
+                        continue;
+                    }
+                    if (d.kind[j] == UFS_CELL_KINETIC && d.kind[q] == UFS_CELL_FLUID) {
+                        m.b_cell.push_back(j); m.b_axis.push_back((int8_t)a); m.b_side.push_back((int8_t)side); m.b_area.push_back(area);
+                        m.b_kind.push_back((int8_t)UFS_BF_FLUID); m.b_state.push_back(q);
+                    }
+                    if (side == 1) {  // interior face, listed once from its low-side cell
+                        m.f_owner.push_back(j); m.f_neigh.push_back(q); m.f_area.push_back(area);
+                        m.f_axis.push_back((int8_t)a); m.f_ratio.push_back((int8_t)((int)d.level[q] - (int)d.level[j]));
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- ghost states: inflow tables (slot order) and fluid-leaf Maxwellian factors -----------------
+    m.n_tables = 0;
+    for (int s = 0; s < 6; s++) {
+        m.table_of_side[s] = -1;
+        if (d.bc[s] != UFS_BC_INFLOW) continue;
+        if (!(d.inflow[s][0] > 0) || !(d.inflow[s][4] > 0)) { err = "inflow state needs n > 0 and T > 0"; return UFS_DVM_EINVAL; }
+        m.table_of_side[s] = m.n_tables++;
+        FluidGhost g;
+        maxwell_factors(d.inflow[s], vel, g);
+        const size_t base = m.tables.size();
+        m.tables.resize(base + vel.Nv);
+        for (int64_t sl = 0; sl < vel.Nv; sl++)
+            m.tables[base + sl] = g.amp * g.g[2][vel.slot_k[sl * 4 + 2]] * g.g[1][vel.slot_k[sl * 4 + 1]] * g.g[0][vel.slot_k[sl * 4 + 0]];
+    }
+    std::vector<int64_t> ghost_of_leaf;
+    if (any_fluid) ghost_of_leaf.assign(n, -1);
+    auto fluid_ghost = [&](int64_t q) -> int64_t {
+        if (ghost_of_leaf[q] < 0) {
+            const double* pm = d.fluid_moments + 5 * q;
+            ghost_of_leaf[q] = (int64_t)m.fluid.size();
+            m.fluid_leaf.push_back(q);
+            m.fluid.emplace_back();
+            maxwell_factors(pm, vel, m.fluid.back());
+        }
+        return ghost_of_leaf[q];
+    };
+
+    // ---- per-cell upwind gather records, derived from the two face lists ---------------------------
+    m.recs.assign(m.n_kin, CellRec{});
+    for (auto& r : m.recs) {
+        for (int dd = 0; dd < 6; dd++) for (int k = 0; k < 4; k++) r.src[dd][k] = -1;
+    }
+    std::vector<int8_t> cnt((size_t)m.n_kin * 6, 0);
+    auto push = [&](int64_t slab, int dir, int32_t code) -> bool {
+        int8_t& c = cnt[(size_t)slab * 6 + dir];
+        if (c >= 4) return false;
+        m.recs[slab].src[dir][c++] = code;
+        return true;
+    };
+    auto code_of = [&](int64_t q) -> int32_t {  // data of leaf q as seen from a kinetic neighbour
+        if (d.kind[q] == UFS_CELL_KINETIC) return src_code(SRC_SLAB, m.slab_of_leaf[q]);
+        return src_code(SRC_FLUID, fluid_ghost(q));
+    };
+    bool ok = true;
+    for (size_t f = 0; f < m.f_owner.size(); f++) {
+        const int64_t p = m.f_owner[f], q = m.f_neigh[f];
+        const int a = m.f_axis[f];
+        if (d.kind[p] == UFS_CELL_KINETIC) {
+            if (d.kind[q] == UFS_CELL_FLUID && !(d.fluid_moments[5 * q] > 0 && d.fluid_moments[5 * q + 4] > 0)) { err = "fluid_moments need n > 0 and T > 0"; return UFS_DVM_EINVAL; }
+            ok &= push(m.slab_of_leaf[p], 2 * a + 1, code_of(q));
+        }
+        if (d.kind[q] == UFS_CELL_KINETIC) {
+            if (d.kind[p] == UFS_CELL_FLUID && !(d.fluid_moments[5 * p] > 0 && d.fluid_moments[5 * p + 4] > 0)) { err = "fluid_moments need n > 0 and T > 0"; return UFS_DVM_EINVAL; }
+            ok &= push(m.slab_of_leaf[q], 2 * a, code_of(p));
+        }
+    }
+    for (size_t b = 0; b < m.b_cell.size(); b++) {
+        const int64_t j = m.b_cell[b];
+        if (d.kind[j] != UFS_CELL_KINETIC || m.b_kind[b] == UFS_BF_FLUID) continue;
+        const int64_t slab = m.slab_of_leaf[j];
+        const int dir = 2 * m.b_axis[b] + m.b_side[b];
+        int32_t code;
+        switch (m.b_kind[b]) {
+            case UFS_BF_SPECULAR: case UFS_BF_SOLID: code = src_code(SRC_MIRROR, slab); break;
+            case UFS_BF_INFLOW: code = src_code(SRC_TABLE, m.table_of_side[m.b_state[b]]); break;
+            default: code = src_code(SRC_SLAB, slab); break;  // outflow: ghost = own cell (zero gradient)
+        }
+        ok &= push(slab, dir, code);
+    }
+    m.n_simple = 0;
+    for (int64_t s = 0; s < m.n_kin; s++) {
+        CellRec& r = m.recs[s];
+        r.level = d.level[m.cell_of_slab[s]];
+        bool simple = true;
+        for (int dd = 0; dd < 6; dd++) {
+            const int c = cnt[(size_t)s * 6 + dd];
+            if (c != 1 && c != 4) ok = false;
+            if (c != 1) simple = false;
+            for (int k = 0; k < c; k++) if ((r.src[dd][k] >> SRC_SHIFT) == SRC_FLUID) simple = false;
+        }
+        r.flags = simple ? CELL_SIMPLE : 0;
+        m.n_simple += simple;
+    }
+    if (!ok) { err = "internal: a kinetic cell has a direction with neither 1 nor 4 sources"; return UFS_DVM_EMESH; }
+    return UFS_DVM_OK;
+}
+
+}  // namespace ufs

@@ -1,0 +1,94 @@
+// flatten.hpp -- host-side octree flattener of the DVM step.
+//
+// Turns the caller's leaf list into what the device kernels consume:
+//   * Morton ("N-order") numbering of the leaves, slabs = kinetic leaves in that order;
+//   * the sorted interior face list (owner, neighbour, area, axis, level ratio) and the boundary-face
+//     list (PAPER.md:51 boundary cells; PAPER.md:207 kinetic/fluid interface);
+//   * per kinetic cell the upwind gather record derived from those faces -- the first-order form of the
+//     paper's per-cell, per-sign-group stencil records m, alpha, a;
+//   * the velocity-slot layout: the 8 sign groups ("octants") stored contiguously.
+// Pure C++, no CUDA.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/ufs_dvm.h"
+
+namespace ufs {
+
+// How a source of upwind data is encoded in a gather record (one int32 per source).
+// code < 0: unused.  Otherwise bits 28..30 = kind, bits 0..27 = index.
+enum SrcKind : int32_t {
+    SRC_SLAB = 0,    // slab `index` of the current f buffer, same velocity slot
+    SRC_MIRROR = 1,  // slab `index` (the cell itself), slot of the velocity mirrored on this axis (specular)
+    SRC_TABLE = 2,   // ghost table `index` (inflow Maxwellian), same slot
+    SRC_FLUID = 3    // fluid ghost `index`: pointwise Maxwellian of frozen moments
+};
+constexpr int32_t SRC_SHIFT = 28;
+constexpr int32_t SRC_INDEX_MASK = (1 << SRC_SHIFT) - 1;
+inline int32_t src_code(SrcKind k, int64_t idx) { return (int32_t)((k << SRC_SHIFT) | (int32_t)idx); }
+
+// One kinetic cell, 128 bytes: for each direction d = 2*axis + side (side 0 = low) up to 4 sources
+// (1 = same level or coarser neighbour / ghost, 4 = finer neighbours, each weighted 1/4).
+struct CellRec {
+    int32_t src[6][4];
+    int32_t level;
+    int32_t flags;  // bit 0: every direction has exactly one source and none is SRC_FLUID
+    int32_t pad[6];
+};
+static_assert(sizeof(CellRec) == 128, "CellRec must be 128 bytes");
+constexpr int32_t CELL_SIMPLE = 1;
+
+constexpr int NV_MAX = 64;  // per-axis node limit (tables live in shared memory)
+
+struct VelLayout {
+    int nv[3];
+    int64_t Nv;
+    double xi[3][NV_MAX];        // node values, canonical index
+    double w;                    // quadrature weight dvx*dvy*dvz (midpoint rule)
+    bool symmetric[3];           // vmin = -vmax on the axis
+    bool fast;                   // every axis: even nv, symmetric => 8 equal octant chunks
+    int nh[3];                   // nv/2 (fast path)
+    int ncls[3][3];              // nodes per sign class (0: xi<0, 1: xi>0, 2: xi==0)
+    std::vector<int32_t> vel_of_slot;      // [Nv] canonical index stored at each slot
+    std::vector<int32_t> slot_of_vel;      // inverse
+    std::vector<int32_t> mirror_slot[3];   // [Nv] slot of the velocity mirrored on axis a (if symmetric[a])
+    std::vector<uint8_t> slot_k;           // [Nv][4] (kx,ky,kz,0) of each slot
+};
+
+struct FluidGhost {          // frozen Maxwellian of a FLUID leaf, separable factors
+    double amp;              // n / (2 pi T)^{3/2}
+    double g[3][NV_MAX];     // exp(-(xi_k - u_a)^2 / 2T), canonical index
+};
+
+struct FlatMesh {
+    int64_t n_leaves = 0, n_kin = 0;
+    int lmax = 0;
+    std::vector<int64_t> order;         // Morton rank -> leaf
+    std::vector<int64_t> rank;          // leaf -> Morton rank
+    std::vector<int64_t> cell_of_slab;  // slab -> leaf
+    std::vector<int64_t> slab_of_leaf;  // leaf -> slab or -1
+    // interior faces (between non-SOLID leaves), sorted by (rank of owner, axis)
+    std::vector<int64_t> f_owner, f_neigh;
+    std::vector<double> f_area;
+    std::vector<int8_t> f_axis, f_ratio;
+    // boundary faces of non-SOLID leaves
+    std::vector<int64_t> b_cell, b_state;
+    std::vector<double> b_area;
+    std::vector<int8_t> b_axis, b_side, b_kind;
+    // device-bound data
+    std::vector<CellRec> recs;          // [n_kin]
+    std::vector<int64_t> fluid_leaf;    // fluid ghost index -> leaf
+    std::vector<FluidGhost> fluid;      // [n fluid ghosts]
+    int table_of_side[6];               // inflow side -> ghost table index or -1
+    int n_tables = 0;
+    std::vector<double> tables;         // [n_tables][Nv] inflow Maxwellians, SLOT order, fp64
+    int64_t n_simple = 0;
+    VelLayout vel;
+};
+
+// Returns UFS_DVM_OK or an error code with a message in `err`.
+int flatten(const ufs_dvm_desc& d, FlatMesh& out, std::string& err);
+
+}  // namespace ufs

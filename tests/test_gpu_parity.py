@@ -1,0 +1,156 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star, reading G17 = max|a-b| / max|b| per array):
+1e-12 for fp64 storage, 2e-5 for fp32 storage with fp64 moment accumulation."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.dvm_oracle import Oracle
+from paper_1503_00707_b200 import binding as B
+from paper_1503_00707_b200 import inputs
+from tests.helpers import periodic_case, random_tree, rel_linf
+
+pytestmark = pytest.mark.gpu
+TOL = {inputs.STORE_F64: 1e-12, inputs.STORE_F32: 2e-5}
+P = (True, True, True)
+
+
+def run_both(case, nsteps, kn=None, storage=None, f0=None):
+    st = B.DvmStepper(case, kn=kn, storage=storage)
+    if f0 is None:
+        f0 = inputs.initial_f(case)
+    if st.storage == inputs.STORE_F32:
+        f0 = f0.astype(np.float32).astype(np.float64)
+    st.load_canonical(f0)
+    st.step(case.dt, nsteps)
+    st.sync()
+    f_gpu = st.read_canonical()
+    m_gpu = st.moments()
+    launches = B.ufs_dvm_launch_count(st.h)
+    info = B.ufs_dvm_kernel_info(st.h)
+    st.close()
+    o = Oracle(case, kn=kn)
+    f_ref = o.step(f0, case.dt, nsteps)
+    m_ref = o.moments(f_ref)
+    return f_gpu, m_gpu, f_ref, m_ref, launches, info
+
+
+def check(case, nsteps, tol, **kw):
+    f_gpu, m_gpu, f_ref, m_ref, launches, info = run_both(case, nsteps, **kw)
+    assert launches == nsteps + 1
+    assert np.all(np.isfinite(f_gpu))
+    err_f = rel_linf(f_gpu, f_ref)
+    assert err_f <= tol, f"f: {err_f:.3e}"
+    for a in range(5):
+        scale = np.abs(m_ref[a]).max()
+        if a in (1, 2, 3):   # a momentum component may vanish (noise only): scale by n * velocity unit sqrt(R T0)
+            scale = max(scale, np.abs(m_ref[0]).max())
+        err = np.abs(m_gpu[a] - m_ref[a]).max() / scale
+        assert err <= tol, f"moment {a}: {err:.3e}"
+    return info
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_small_configs_match_oracle(cfg):
+    case = inputs.small(cfg)
+    info = check(case, case.nsteps, TOL[case.storage])
+    assert info["fast"]
+
+
+def test_config1_full_run_10_steps():
+    case = inputs.config1()
+    check(case, 10, 1e-12)
+
+
+def test_config1_fp32_storage():
+    case = inputs.config1()
+    check(case, 10, 2e-5, storage=inputs.STORE_F32)
+
+
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_transport_only_kn_inf(cfg):
+    case = inputs.small(cfg)
+    check(case, 3, 1e-13, kn=math.inf)
+
+
+def test_small_config3_fp32():
+    case = inputs.small(3)
+    check(case, 3, 2e-5, storage=inputs.STORE_F32)
+
+
+def test_small_config5_fp32():
+    case = inputs.small(5)
+    check(case, 3, 2e-5, storage=inputs.STORE_F32)
+
+
+@pytest.mark.parametrize("nv,vmin,vmax", [((5, 4, 3), (-4.0, -3.0, -2.5), (4.0, 5.0, 2.5)),
+                                          ((7, 7, 7), (-4.0,) * 3, (4.0,) * 3),
+                                          ((6, 10, 2), (-4.0, -5.0, -2.0), (4.0, 5.0, 2.0))])
+def test_generic_and_odd_velocity_grids(nv, vmin, vmax):
+    """Odd nv (a zero node carries no flux on its axis), asymmetric limits, non-cubic grids."""
+    lv, ijk = random_tree(np.random.default_rng(4), 1, 3, P, 0.3)
+    case = periodic_case(lv, ijk, nv=nv, kn=0.2)
+    case.vmin, case.vmax = vmin, vmax
+    rng = np.random.default_rng(1)
+    f0 = inputs.maxwellian_canonical(case, case.prim0) * (1 + 0.2 * rng.uniform(-1, 1, (case.n_leaves, case.Nv)))
+    info = check(case, 3, 1e-12, f0=f0)
+    sym_even = all(n % 2 == 0 and abs(a + b) < 1e-12 for n, a, b in zip(nv, vmin, vmax))
+    assert info["fast"] == sym_even
+
+
+def test_specular_box_with_odd_grid_generic_path():
+    lv, ijk = inputs.build_tree(2, 2, {}, P)
+    case = periodic_case(lv, ijk, nv=(5, 5, 5), bc=(inputs.BC_SPECULAR,) * 6, kn=0.3)
+    rng = np.random.default_rng(2)
+    f0 = inputs.maxwellian_canonical(case, case.prim0) * (1 + 0.2 * rng.uniform(-1, 1, (case.n_leaves, case.Nv)))
+    check(case, 3, 1e-12, f0=f0)
+
+
+def test_newton_failure_is_reported():
+    case = inputs.config1()
+    st = B.DvmStepper(case)
+    f0 = -inputs.initial_f(case)                     # negative density
+    st.load_canonical(f0)
+    st.step(case.dt, 1)
+    with pytest.raises(B.UfsDvmError) as e:
+        st.sync()
+    assert e.value.code == B.ENEWTON
+    with pytest.raises(B.UfsDvmError):               # sticky
+        st.step(case.dt, 1)
+    st.close()
+
+
+def test_run_host_entry_point():
+    import ctypes as C
+    import torch
+    case = inputs.small(2)
+    st = B.DvmStepper(case)
+    f0 = inputs.initial_f(case)
+    host_in = np.ascontiguousarray(f0[st.row_of_slab][:, st.vel_of_slot])
+    host_out = np.empty_like(host_in)
+    mom_host = np.empty((5, st.n_kinetic))
+    B.ufs_dvm_run_host(st.h, host_in.ctypes.data, host_out.ctypes.data, st.mom.data_ptr(), mom_host.ctypes.data,
+                       case.dt, 2)
+    o = Oracle(case)
+    f_ref = o.step(f0, case.dt, 2)
+    inv = np.empty(case.Nv, np.int64); inv[st.vel_of_slot] = np.arange(case.Nv)
+    got = np.empty_like(f_ref); got[st.row_of_slab] = host_out[:, inv]
+    assert rel_linf(got, f_ref) <= 1e-12
+    m = np.empty_like(mom_host); m[:, st.row_of_slab] = mom_host
+    assert rel_linf(m[0], o.moments(f_ref)[0]) <= 1e-12
+    st.close()
+
+
+def test_uniform_maxwellian_steady_on_gpu():
+    """P1 on the device: adaptive periodic tree, same Maxwellian everywhere, collisions on."""
+    case = inputs.config1(nv=24)
+    case.vmin, case.vmax = (-5.0,) * 3, (5.0,) * 3
+    prim = np.tile(np.array([[1.3, 0.4, -0.2, 0.1, 0.9]]), (case.n_leaves, 1))
+    f0 = inputs.maxwellian_canonical(case, prim)
+    st = B.DvmStepper(case)
+    st.load_canonical(f0)
+    st.step(case.dt, 3)
+    st.sync()
+    assert rel_linf(st.read_canonical(), f0) < 5e-14
+    st.close()
