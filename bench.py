@@ -1,0 +1,241 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused DVM step on B200 (one JSON line on stdout).
+
+metric: phase-space cell updates per second (N_kinetic * Nv * steps / time), BASELINE.json.
+Workload (N=1): the configuration the north-star target is stated on -- the ~1.0e6-leaf periodic
+octree with a 24^3 velocity grid, fp32 storage, fp64 moment accumulation (BASELINE.json configs[3],
+SURVEY.md 8(d) row 4); both f buffers (2 x 55.8 GB) resident in HBM.  Synthetic, seeded inputs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3]
+    python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
+
+N > 1 runs N independent replicas (the path is one GPU by the north star).
+"""
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "phase-space cell updates/s per DVM step"
+UNIT = "updates/s"
+
+
+def make_case(workload: str):
+    from paper_1503_00707_b200 import inputs
+    if workload == "config4":
+        return inputs.config4()
+    if workload == "config4_lit":
+        return inputs.config4(target_leaves=None)
+    if workload == "config4_small":      # the same recipe one level coarser (ncu captures, quick looks)
+        return inputs.config4(base=5, lmax=7, target_leaves=125_000, side_scale=2.0)
+    if workload == "config2":
+        return inputs.config2()
+    if workload == "config3":
+        return inputs.config3(lmax=8)
+    raise SystemExit(f"unknown workload {workload}")
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json, copy bandwidth)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic_ratio(workload: str):
+    """DRAM bytes per algorithmic byte of the step kernel from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "step_kernel_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    best = None
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            w, storage, alg, rd, wr = line.strip().split(",")[:5]
+            if w.startswith(workload.split("_")[0]):
+                best = (float(rd) + float(wr)) / float(alg)
+    return best
+
+
+def oracle_sample(case, n_sample: int):
+    """A bounded sample of the workload for the CPU oracle: the window made of the first n_sample
+    leaves in Morton order (missing neighbours at the window edge become zero-gradient ghosts)."""
+    from paper_1503_00707_b200 import binding as B
+    from paper_1503_00707_b200 import harness
+    desc, keep = B.make_desc(case)
+    h = B.ufs_dvm_create_host(desc)
+    _, cell_of_slab, _ = B.ufs_dvm_layout(h, case.Nv)
+    B.ufs_dvm_destroy(h)
+    ids = np.sort(cell_of_slab[:n_sample])
+    return harness.sub_case(case, ids, case.name + "_sample")
+
+
+def time_oracle(case, n_sample: int, steps: int, warmup: int):
+    from oracle import dvm_oracle
+    from paper_1503_00707_b200 import inputs
+    sub = oracle_sample(case, n_sample)
+    o = dvm_oracle.Oracle(sub, window=True)
+    f = inputs.initial_f(sub)
+    for _ in range(warmup):
+        f = o.step(f, case.dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        f = o.step(f, case.dt)
+    t = time.perf_counter() - t0
+    units = o.n_kinetic * sub.Nv * steps
+    return {"value": units / t, "unit": UNIT, "cores": dvm_oracle.threads(), "kind": "oracle",
+            "sample": f"window of the first {o.n_kinetic} Morton-ordered leaves of {case.name}, {steps} steps "
+                      f"(fp64, OpenMP over cells)", "seconds": t}, t / steps
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    case = make_case(args.workload)
+    n_sample = args.oracle_leaves or 4096
+    base, ms = time_oracle(case, n_sample, max(1, args.steps), args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(case, args),
+            "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(case, args):
+    return {"workload": f"{args.workload}: {case.name}, {int((case.kind == 0).sum())} kinetic leaves "
+                        f"(levels {int(case.level.min())}-{int(case.level.max())}), velocity grid "
+                        f"{case.nv[0]}x{case.nv[1]}x{case.nv[2]} on [{case.vmin[0]},{case.vmax[0]}]^3, Kn {case.kn}, CFL {case.cfl}",
+            "storage": "fp32" if case.storage == 1 else "fp64",
+            "l2": "inputs larger than L2 (f buffers far exceed 126 MB); no flush needed",
+            "parallelism": "1 GPU" if args.gpus == 1 else f"{args.gpus} independent replicas"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4")
+    ap.add_argument("--oracle-leaves", type=int, default=0, help="size of the CPU-oracle sample (0 = default)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1503_00707_b200 import binding as B
+    from paper_1503_00707_b200 import harness
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the DVM step has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    case = make_case(args.workload)
+    st = B.DvmStepper(case, device=dev)
+    harness.fill_initial_f_device(st, case)
+    torch.cuda.synchronize(dev)
+    n_kin, Nv = st.n_kinetic, st.Nv
+    elem = 4 if case.storage == 1 else 8
+    dt = case.dt
+    info = B.ufs_dvm_kernel_info(st.h)
+
+    # ---- end-to-end leg first (it restarts from f0): host buffers through ufs_dvm_run_host ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            host_in = torch.empty((n_kin, Nv), dtype=st.dtype, pin_memory=True)
+            host_in.copy_(st.f[B.ufs_dvm_current(st.h)])
+            mom_host = torch.empty((5, n_kin), dtype=torch.float64, pin_memory=True)
+            B.ufs_dvm_run_host(st.h, host_in.data_ptr(), None, st.mom.data_ptr(), mom_host.data_ptr(), dt, 1)  # warm
+            barrier()
+            t0 = time.perf_counter()
+            B.ufs_dvm_run_host(st.h, host_in.data_ptr(), None, st.mom.data_ptr(), mom_host.data_ptr(), dt, args.steps)
+            torch.cuda.synchronize(dev)
+            t_e2e = time.perf_counter() - t0
+            if world > 1:
+                tt = torch.tensor([t_e2e], device=dev); dist.all_reduce(tt, op=dist.ReduceOp.MAX); t_e2e = float(tt.item())
+            e2e = {"value": world * n_kin * Nv * args.steps / t_e2e, "unit": UNIT,
+                   "h2d_bytes_per_step": n_kin * Nv * elem / args.steps, "d2h_bytes_per_step": n_kin * 40 / args.steps,
+                   "seconds": t_e2e,
+                   "what": "ufs_dvm_run_host: pinned host f -> device, K steps, moments, moments -> host"}
+            del host_in
+        except Exception as ex:  # host memory too small for a pinned copy of f, etc.
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                   "unavailable": f"{type(ex).__name__}: {ex}"[:200]}
+        harness.fill_initial_f_device(st, case)
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events ----
+    st.step(dt, args.warmup)
+    barrier()
+    launches0 = B.ufs_dvm_launch_count(st.h)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with harness.ClockSampler(index=torch.cuda.current_device()) as clk:
+        ev0.record(st.stream)
+        st.step(dt, args.steps)
+        ev1.record(st.stream)
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = B.ufs_dvm_launch_count(st.h) - launches0
+    st.sync()                                   # raises on a sticky CUDA / Newton error
+    if world > 1:
+        tt = torch.tensor([ms], device=dev); dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = float(tt.item())
+    updates = n_kin * Nv * args.steps
+    value = world * updates / (ms * 1e-3)
+
+    # ---- roofline of the (only) kernel in the step ----
+    peak, peak_src = peaks()
+    alg_bytes_per_launch = 2.0 * n_kin * Nv * elem          # 1 read + 1 write of f per phase-space cell
+    achieved = alg_bytes_per_launch / (ms * 1e-3 / args.steps) / 1e9
+    ratio = ncu_traffic_ratio(args.workload)
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None if ratio is None else ratio * alg_bytes_per_launch,
+                "peak_source": peak_src, "kernel": "k_step_fast" if info["fast"] else "k_step_generic",
+                "algorithmic_bytes_per_launch": alg_bytes_per_launch,
+                "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if case.storage == 1 else "f64", "data": "synthetic",
+            "config": workload_config(case, args), "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "kernel": info}
+
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        st.close(); del st
+        torch.cuda.empty_cache()
+        base, _ = time_oracle(case, args.oracle_leaves or 16384, 2, 0)
+        line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
