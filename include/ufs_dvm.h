@@ -83,7 +83,9 @@ int ufs_dvm_create(const ufs_dvm_desc *desc, void *f_dev[2], void *cuda_stream, 
 int ufs_dvm_create_host(const ufs_dvm_desc *desc, ufs_dvm_t *out);
 
 /* Enqueue nsteps explicit steps of size dt (transport -> moments -> discrete Maxwellian -> BGK
- * relaxation, one fused kernel per step).  f ping-pongs between the two buffers. */
+ * relaxation, one fused kernel per step).  f ping-pongs between the two buffers.  The environment
+ * variable UFS_DVM_KERNEL=cell (read by ufs_dvm_create) selects the one-CTA-per-cell kernels even where
+ * the persistent ring kernel applies. */
 int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps);
 
 /* Enqueue the moments of the current f: mom_dev is DEVICE memory, [5][n_kinetic] doubles in slab order:
@@ -129,6 +131,10 @@ int64_t ufs_dvm_launch_count(ufs_dvm_t h);
 /* Launch geometry of the step kernel: threads per CTA, dynamic shared memory per CTA, vector width in
  * elements, and 1 if the octant fast path is used (0 = generic per-slot path).  HOST outputs. */
 int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t *threads, int32_t *smem_bytes, int32_t *vec, int32_t *fast);
+
+/* Name of the step kernel this handle launches: "k_step_ring" (persistent TMA ring kernel),
+ * "k_step_fast" (one CTA per cell, octant layout) or "k_step_generic" (any velocity grid).  Never NULL. */
+const char *ufs_dvm_kernel_name(ufs_dvm_t h);
 
 /* Message of the last error on this handle (valid until the next call on it); never NULL. */
 const char *ufs_dvm_last_error(ufs_dvm_t h);

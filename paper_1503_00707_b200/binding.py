@@ -19,7 +19,8 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
-           "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_last_error"]
+           "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
+           "ufs_dvm_last_error"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -59,6 +60,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
+        L.ufs_dvm_kernel_name.argtypes = [vp]; L.ufs_dvm_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -177,6 +179,10 @@ def ufs_dvm_kernel_info(h) -> dict:
     t, s, v, f = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
     _check(h, lib().ufs_dvm_kernel_info(h, C.byref(t), C.byref(s), C.byref(v), C.byref(f)))
     return {"threads": t.value, "smem_bytes": s.value, "vec": v.value, "fast": bool(f.value)}
+
+
+def ufs_dvm_kernel_name(h) -> str:
+    return lib().ufs_dvm_kernel_name(h).decode()
 
 
 def ufs_dvm_last_error(h) -> str:

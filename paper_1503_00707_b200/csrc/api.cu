@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libufs_dvm.so (include/ufs_dvm.h): handle life cycle, uploads of what the
 // flattener built, and the enqueue calls.  No torch types, no exceptions across the boundary.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -26,6 +27,9 @@ struct ufs_dvm_s {
     uchar4* d_slot_k = nullptr;
     int32_t* d_mirror = nullptr;
     int32_t* d_flags = nullptr;
+    int32_t* d_counter = nullptr;  // [2] cell counters of the ring kernel, one per launch parity
+    int parity = 0;
+    int l2_mode = 0;
     StepLaunch plan{};
     int64_t launches = 0;
     int sticky = UFS_DVM_OK;
@@ -79,6 +83,10 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.inv_kn = p.collide ? 1.0 / h->kn : 0.0;
     p.visc_exp = h->visc_exp;
     p.nu_pref = h->nu_pref;
+    p.counter = h->d_counter + h->parity;
+    p.counter_reset = h->d_counter + (h->parity ^ 1);
+    p.ring_stages = h->plan.stages;
+    p.l2_mode = h->l2_mode;
     return p;
 }
 
@@ -146,6 +154,25 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     if ((rc = upload(h, &h->d_tables, tab, tab_bytes, "upload inflow tables"))) return rc;
     CU(cudaMalloc(reinterpret_cast<void**>(&h->d_flags), 4), "allocate flags");
     CU(cudaMemsetAsync(h->d_flags, 0, 4, h->stream), "clear flags");
+    CU(cudaMalloc(reinterpret_cast<void**>(&h->d_counter), 8), "allocate cell counters");
+    CU(cudaMemsetAsync(h->d_counter, 0, 8, h->stream), "clear cell counters");
+    // kernel choice: the persistent TMA ring kernel where the velocity grid fits it, else one CTA per cell
+    // (UFS_DVM_KERNEL=cell forces the latter: A/B timing and tests)
+    if (const char* l2 = std::getenv("UFS_DVM_L2")) h->l2_mode = std::atoi(l2);
+    const char* force = std::getenv("UFS_DVM_KERNEL");
+    if (!(force && std::strcmp(force, "cell") == 0)) {
+        int dev = 0, sms = 0;
+        CU(cudaGetDevice(&dev), "get device");
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
+        StepLaunch ring{};
+        if (ring_plan(h->storage, v, sms, &ring)) {
+            const int occ = ring_occupancy(h->storage, ring);
+            if (occ > 0) {
+                ring.grid = sms * occ;
+                h->plan = ring;
+            }
+        }
+    }
     CU(cudaStreamSynchronize(h->stream), "upload");  // the host vectors above die at return
     return UFS_DVM_OK;
 }
@@ -159,6 +186,7 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
         const StepParams p = make_params(h, dt);
         CU(launch_step(h->storage, h->plan, p, h->stream), "step kernel launch");
         h->cur ^= 1;
+        h->parity ^= 1;
         if (h->mesh.n_kin > 0) h->launches++;
     }
     return UFS_DVM_OK;
@@ -194,7 +222,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
     if (h->device) {
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) rc = UFS_DVM_ECUDA;
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
-        cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags);
+        cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
     }
     delete h;
     return rc;
@@ -263,6 +291,11 @@ int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int3
     if (vec) *vec = h->plan.vec;
     if (fast) *fast = h->plan.fast;
     return UFS_DVM_OK;
+}
+
+const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
+    if (!h) return "";
+    return h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
 }
 
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }

@@ -64,11 +64,6 @@ struct Smem {
     const void** ptr;     // [8][4] per octant: own chunk, x/y/z upwind chunk (simple cells)
     int* rec;             // [32] the cell record
 };
-__host__ __device__ inline int nvp_of(const int32_t nv[3]) {
-    int m = nv[0] > nv[1] ? nv[0] : nv[1];
-    m = m > nv[2] ? m : nv[2];
-    return (m + 3) & ~3;
-}
 __host__ __device__ inline size_t smem_bytes_for(int64_t Nv, size_t elem, int nvp, int nwarps) {
     size_t b = ((size_t)Nv * elem + 15) & ~(size_t)15;
     b += (size_t)nwarps * 5 * 8 + 4 * 8 + (size_t)3 * nvp * 8 + (size_t)3 * nvp * 4 + 32 * 8 + 32 * 4;
@@ -546,6 +541,8 @@ cudaError_t launch_generic(const StepLaunch& plan, const StepParams& p, cudaStre
 int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** why) {
     const size_t elem = storage == UFS_STORE_F32 ? 4 : 8;
     const int nvp = nvp_of(v.nv);
+    plan->ring = 0;
+    plan->grid = plan->ncw = plan->pieces = plan->stages = 0;
     plan->fast = v.fast ? 1 : 0;
     plan->vec = 1;
     int threads = 256;
@@ -572,6 +569,7 @@ int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** wh
 
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
     if (p.n_kin == 0) return cudaSuccess;
+    if (plan.ring) return launch_ring(storage, plan, p, st);
     if (plan.fast) {
         if (storage == UFS_STORE_F32) {
             if (plan.vec == 4) return launch_fast<float, 4>(plan, p, st);

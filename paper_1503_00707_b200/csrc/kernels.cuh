@@ -31,15 +31,34 @@ struct StepParams {
     int32_t nv[3], nh[3];
     int32_t collide;            // 0: Kn = inf, pure transport
     double dt, w, inv_len, inv_kn, visc_exp, nu_pref;
+    int32_t* counter;           // ring kernel: cell counter of this launch (zero at launch)
+    int32_t* counter_reset;     // ring kernel: the other launch parity's counter, zeroed by this launch
+    int32_t ring_stages;        // ring kernel: stages in the shared-memory ring
+    int32_t l2_mode;            // ring kernel: L2 eviction hints on the bulk loads (0 none; see step_ring.cu)
 };
 
 struct StepLaunch {
     int32_t threads, smem_bytes, vec, fast;
+    int32_t ring;                  // 1: persistent TMA ring kernel (step_ring.cu), 0: one CTA per cell (kernels.cu)
+    int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
 };
+
+// per-axis table stride (nodes rounded up to a multiple of 4)
+__host__ __device__ inline int nvp_of(const int32_t nv[3]) {
+    int m = nv[0] > nv[1] ? nv[0] : nv[1];
+    m = m > nv[2] ? m : nv[2];
+    return (m + 3) & ~3;
+}
 
 // Chooses the kernel variant for this storage type / grid and returns its launch geometry, or an
 // error (negative) if the slab does not fit on chip.
 int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** why);
+
+// step_ring.cu: geometry of the persistent TMA ring kernel for this storage type / grid (false: not
+// applicable), and its launcher.
+bool ring_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
+int ring_occupancy(int storage, const StepLaunch& plan);
+cudaError_t launch_ring(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
