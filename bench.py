@@ -130,6 +130,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4")
     ap.add_argument("--oracle-leaves", type=int, default=0, help="size of the CPU-oracle sample (0 = default)")
+    ap.add_argument("--kn", type=float, default=None, help="override the Knudsen number (inf = collisions off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -157,6 +158,8 @@ def main():
         torch.cuda.synchronize(dev)
 
     case = make_case(args.workload)
+    if args.kn is not None:
+        case.kn = args.kn
     st = B.DvmStepper(case, device=dev)
     harness.fill_initial_f_device(st, case)
     torch.cuda.synchronize(dev)
@@ -164,6 +167,7 @@ def main():
     elem = 4 if case.storage == 1 else 8
     dt = case.dt
     info = B.ufs_dvm_kernel_info(st.h)
+    kernel_name = B.ufs_dvm_kernel_name(st.h)
 
     # ---- end-to-end leg first (it restarts from f0): host buffers through ufs_dvm_run_host ----
     e2e = None
@@ -216,7 +220,7 @@ def main():
     ratio = ncu_traffic_ratio(args.workload)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None if ratio is None else ratio * alg_bytes_per_launch,
-                "peak_source": peak_src, "kernel": "k_step_fast" if info["fast"] else "k_step_generic",
+                "peak_source": peak_src, "kernel": kernel_name,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch,
                 "frac_of_8TBs_nominal": achieved / 8000.0}
 
