@@ -30,6 +30,7 @@ struct ufs_dvm_s {
     int32_t* d_counter = nullptr;  // [2] cell counters of the ring kernel, one per launch parity
     int parity = 0;
     int l2_mode = 0;
+    int ticket_mode = 1;
     StepLaunch plan{};
     int64_t launches = 0;
     int sticky = UFS_DVM_OK;
@@ -87,6 +88,7 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.counter_reset = h->d_counter + (h->parity ^ 1);
     p.ring_stages = h->plan.stages;
     p.l2_mode = h->l2_mode;
+    p.ticket_mode = h->ticket_mode;
     return p;
 }
 
@@ -159,6 +161,7 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     // kernel choice: the persistent TMA ring kernel where the velocity grid fits it, else one CTA per cell
     // (UFS_DVM_KERNEL=cell forces the latter: A/B timing and tests)
     if (const char* l2 = std::getenv("UFS_DVM_L2")) h->l2_mode = std::atoi(l2);
+    if (const char* tk = std::getenv("UFS_DVM_TICKET")) h->ticket_mode = std::atoi(tk);
     const char* force = std::getenv("UFS_DVM_KERNEL");
     if (!(force && std::strcmp(force, "cell") == 0)) {
         int dev = 0, sms = 0;

@@ -35,6 +35,7 @@ struct StepParams {
     int32_t* counter_reset;     // ring kernel: the other launch parity's counter, zeroed by this launch
     int32_t ring_stages;        // ring kernel: stages in the shared-memory ring
     int32_t l2_mode;            // ring kernel: L2 eviction hints on the bulk loads (0 none; see step_ring.cu)
+    int32_t ticket_mode;        // ring kernel: how cells are handed to CTAs (see step_ring.cu)
 };
 
 struct StepLaunch {

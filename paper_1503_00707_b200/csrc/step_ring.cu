@@ -324,8 +324,13 @@ __global__ void __launch_bounds__((NCW + 1) * 32, MINB) k_step_ring(const StepPa
         auto load_rec = [&](int cell) -> int {
             return cell < p.n_kin ? __ldg(reinterpret_cast<const int*>(p.cells + cell) + lane) : 0;
         };
-        int cur = __shfl_sync(0xffffffffu, fetch_async(), 0);
-        int nxt_raw = fetch_async();
+        // ticket_mode 0: the next cell's ticket is drawn while the current cell starts (its record is in
+        // flight during the copies); 1: drawn when the current cell's last octant is issued, so that the
+        // cells in flight stay consecutive in slab order; 2: static round-robin over the grid
+        const int tm = p.ticket_mode;
+        auto next_ticket = [&](int c) -> int { return tm == 2 ? c + (int)gridDim.x : fetch_async(); };
+        int cur = tm == 2 ? (int)blockIdx.x : __shfl_sync(0xffffffffu, fetch_async(), 0);
+        int nxt_raw = tm == 1 ? 0 : next_ticket(cur);
         int rec = load_rec(cur);
         const int o_l = lane >> 2, t_l = lane & 3;
         // L2 policy of this lane's stream.  Every chunk is read four times per step (by its own cell and by
@@ -348,9 +353,12 @@ __global__ void __launch_bounds__((NCW + 1) * 32, MINB) k_step_ring(const StepPa
                 if (lane == 0) { s.info[slot] = make_int4(0, 0, RING_STOP, 0); mbar_arrive(&s.full[slot]); }
                 break;
             }
-            const int nxt = __shfl_sync(0xffffffffu, nxt_raw, 0);
-            nxt_raw = fetch_async();
-            const int nrec = load_rec(nxt);  // in flight while this cell's copies are issued
+            int nxt = 0, nrec = 0;
+            if (tm != 1) {
+                nxt = __shfl_sync(0xffffffffu, nxt_raw, 0);
+                nxt_raw = next_ticket(nxt);
+                nrec = load_rec(nxt);  // in flight while this cell's copies are issued
+            }
             const int level = __shfl_sync(0xffffffffu, rec, 24), flags = __shfl_sync(0xffffffffu, rec, 25);
             if (flags & CELL_SIMPLE) {
                 // lane (o,t): stream t of octant o -- t = 0 own chunk, t = 1..3 the upwind chunk on axis t-1
@@ -363,6 +371,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, MINB) k_step_ring(const StepPa
                                           : (kind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + idx * p.Nv
                                                 + (int64_t)(kind == SRC_MIRROR ? (o_l ^ (1 << a)) : o_l) * CH;
                 for (int o = 0; o < 8; o++) {
+                    if (tm == 1 && o == 7) nxt_raw = fetch_async();
 #pragma unroll
                     for (int q = 0; q < PIECES; q++) {
                         mbar_wait(&s.empty[slot], ph ^ 1u);
@@ -380,9 +389,14 @@ __global__ void __launch_bounds__((NCW + 1) * 32, MINB) k_step_ring(const StepPa
                     }
                 }
             } else {
+                if (tm == 1) nxt_raw = fetch_async();
                 mbar_wait(&s.empty[slot], ph ^ 1u);
                 if (lane == 0) { s.info[slot] = make_int4(cur, level, RING_GATHER, 0); mbar_arrive(&s.full[slot]); }
                 advance();
+            }
+            if (tm == 1) {
+                nxt = __shfl_sync(0xffffffffu, nxt_raw, 0);
+                nrec = load_rec(nxt);
             }
             cur = nxt;
             rec = nrec;
