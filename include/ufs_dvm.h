@@ -101,6 +101,13 @@ int ufs_dvm_destroy(ufs_dvm_t h);
 /* 0 or 1: which of f_dev[] holds the current f. */
 int ufs_dvm_current(ufs_dvm_t h);
 
+/* Tell the library that the caller has (re)written the current f buffer on the device.  The streaming step keeps,
+ * per cell, 35 velocity sums of the current f (the moments of Eq. 2's upwind fluxes, that the next
+ * step's Maxwellian needs) from one step to the next; after this call they are recomputed from f by one extra
+ * pass at the next ufs_dvm_step / ufs_dvm_moments.  Not needed after ufs_dvm_create (nothing is cached yet) nor
+ * with ufs_dvm_run_host (it does this itself).  Host-side flag only; returns UFS_DVM_OK. */
+int ufs_dvm_f_changed(ufs_dvm_t h);
+
 /* Layout of the f buffers (HOST outputs, any may be NULL): *n_kinetic; cell_of_slab[n_kinetic] = index into
  * the caller's leaf list; vel_of_slot[Nv] = canonical velocity index (kz*nv[1] + ky)*nv[0] + kx stored at
  * each slab slot.  Slabs are in Morton order, slots grouped by velocity octant. */

@@ -20,7 +20,7 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
-           "ufs_dvm_last_error"]
+           "ufs_dvm_last_error", "ufs_dvm_f_changed"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -53,6 +53,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_sync.argtypes = [vp]
         L.ufs_dvm_destroy.argtypes = [vp]
         L.ufs_dvm_current.argtypes = [vp]
+        L.ufs_dvm_f_changed.argtypes = [vp]
         L.ufs_dvm_layout.argtypes = [vp, C.POINTER(C.c_int64), i64p, vp]
         L.ufs_dvm_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp]
         L.ufs_dvm_boundary_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
@@ -133,6 +134,10 @@ def ufs_dvm_destroy(h):
 
 def ufs_dvm_current(h) -> int:
     return int(lib().ufs_dvm_current(h))
+
+
+def ufs_dvm_f_changed(h):
+    _check(h, lib().ufs_dvm_f_changed(h))
 
 
 def ufs_dvm_layout(h, Nv: int):
@@ -231,6 +236,7 @@ class DvmStepper:
             rows = self.row_of_slab[s0:s0 + chunk]
             part = f_rows[rows][:, self.vel_of_slot]
             self.f[cur][s0:s0 + chunk].copy_(torch.from_numpy(np.ascontiguousarray(part)).to(self.dtype))
+        ufs_dvm_f_changed(self.h)
 
     def read_canonical(self, slabs: Optional[np.ndarray] = None) -> np.ndarray:
         """Current f as float64 [rows, Nv] in canonical order.  With `slabs`, only those slabs, in the

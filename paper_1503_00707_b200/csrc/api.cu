@@ -28,6 +28,11 @@ struct ufs_dvm_s {
     int32_t* d_mirror = nullptr;
     int32_t* d_flags = nullptr;
     int32_t* d_counter = nullptr;  // [2] cell counters of the ring kernel, one per launch parity
+    // streaming step: velocity sums of f[0] / f[1], of the ghost states, and the per-step factor tables
+    double* d_sums[2] = {nullptr, nullptr};
+    double* d_ghost_sums = nullptr;
+    void* d_tabs = nullptr;
+    bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
     int l2_mode = 0;
     int ticket_mode = 1;
@@ -89,7 +94,30 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.ring_stages = h->plan.stages;
     p.l2_mode = h->l2_mode;
     p.ticket_mode = h->ticket_mode;
+    p.sums_in = h->d_sums[h->cur];
+    p.sums_out = h->d_sums[h->cur ^ 1];
+    p.ghost_sums = h->d_ghost_sums;
+    p.tabs = h->d_tabs;
+    p.n_tables = h->mesh.n_tables;
     return p;
+}
+
+// The 35 velocity sums (layout of step_stream.cu: H[5], then G[axis][sign][5]) of one ghost state given by its
+// values in slot order, exactly as the step kernel sees them (storage-type rounding included).
+template <typename F>
+void ghost_state_sums(const VelLayout& v, F value_of_slot, double* out) {
+    for (int i = 0; i < SUMS_STRIDE; i++) out[i] = 0.0;
+    for (int64_t sl = 0; sl < v.Nv; sl++) {
+        const double x[3] = {v.xi[0][v.slot_k[sl * 4]], v.xi[1][v.slot_k[sl * 4 + 1]], v.xi[2][v.slot_k[sl * 4 + 2]]};
+        const double m[5] = {1.0, x[0], x[1], x[2], x[0] * x[0] + x[1] * x[1] + x[2] * x[2]};
+        const double f = value_of_slot(sl);
+        for (int k = 0; k < 5; k++) out[k] += m[k] * f;
+        for (int a = 0; a < 3; a++) {
+            if (x[a] == 0.0) continue;
+            const int s = x[a] > 0.0 ? 1 : 0;
+            for (int k = 0; k < 5; k++) out[5 + (2 * a + s) * 5 + k] += m[k] * std::fabs(x[a]) * f;
+        }
+    }
 }
 
 int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out) {
@@ -162,19 +190,49 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     // (UFS_DVM_KERNEL=cell forces the latter: A/B timing and tests)
     if (const char* l2 = std::getenv("UFS_DVM_L2")) h->l2_mode = std::atoi(l2);
     if (const char* tk = std::getenv("UFS_DVM_TICKET")) h->ticket_mode = std::atoi(tk);
+    // UFS_DVM_KERNEL = stream (default) | ring | cell : A/B timing and tests of the older kernels
     const char* force = std::getenv("UFS_DVM_KERNEL");
-    if (!(force && std::strcmp(force, "cell") == 0)) {
+    const bool want_cell = force && std::strcmp(force, "cell") == 0;
+    const bool want_ring = force && std::strcmp(force, "ring") == 0;
+    if (!want_cell) {
         int dev = 0, sms = 0;
         CU(cudaGetDevice(&dev), "get device");
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
-        StepLaunch ring{};
-        if (ring_plan(h->storage, v, sms, &ring)) {
-            const int occ = ring_occupancy(h->storage, ring);
+        StepLaunch cand{};
+        if (!want_ring && stream_plan(h->storage, v, sms, &cand)) {
+            h->plan = cand;
+        } else if (ring_plan(h->storage, v, sms, &cand)) {
+            const int occ = ring_occupancy(h->storage, cand);
             if (occ > 0) {
-                ring.grid = sms * occ;
-                h->plan = ring;
+                cand.grid = sms * occ;
+                h->plan = cand;
             }
         }
+    }
+    if (h->plan.ring == 2 && m.n_kin > 0) {
+        const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
+        const size_t sums_bytes = (size_t)m.n_kin * SUMS_STRIDE * sizeof(double);
+        for (int b = 0; b < 2; b++) CU(cudaMalloc(reinterpret_cast<void**>(&h->d_sums[b]), sums_bytes), "allocate velocity sums");
+        CU(cudaMalloc(&h->d_tabs, (size_t)m.n_kin * stream_tabn(v) * elem), "allocate factor tables");
+        // sums of the ghost states (inflow tables, fluid leaves), from the values the kernel will read
+        const size_t ng = (size_t)m.n_tables + m.fluid.size();
+        std::vector<double> gs(ng * SUMS_STRIDE);
+        const bool f32 = h->storage == UFS_STORE_F32;
+        for (int t = 0; t < m.n_tables; t++) {
+            const double* tb = m.tables.data() + (size_t)t * v.Nv;
+            ghost_state_sums(v, [&](int64_t sl) { return f32 ? (double)(float)tb[sl] : tb[sl]; }, gs.data() + (size_t)t * SUMS_STRIDE);
+        }
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t g = 0; g < (int64_t)m.fluid.size(); g++) {
+            const FluidGhost& fg = m.fluid[g];
+            ghost_state_sums(v, [&](int64_t sl) {
+                const double b = fg.amp * fg.g[2][v.slot_k[sl * 4 + 2]] * fg.g[1][v.slot_k[sl * 4 + 1]];
+                const double val = b * fg.g[0][v.slot_k[sl * 4]];
+                return f32 ? (double)(float)val : val;
+            }, gs.data() + ((size_t)m.n_tables + g) * SUMS_STRIDE);
+        }
+        if ((rc = upload(h, &h->d_ghost_sums, gs.data(), gs.size() * sizeof(double), "upload ghost sums"))) return rc;
+        CU(cudaStreamSynchronize(h->stream), "upload");  // gs dies at the end of this block
     }
     CU(cudaStreamSynchronize(h->stream), "upload");  // the host vectors above die at return
     return UFS_DVM_OK;
@@ -185,12 +243,19 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!(dt > 0) || nsteps < 0) return fail(h, UFS_DVM_EINVAL, "dt must be positive and nsteps >= 0");
+    const bool stream = h->plan.ring == 2 && h->mesh.n_kin > 0;
     for (int s = 0; s < nsteps; s++) {
         const StepParams p = make_params(h, dt);
+        if (stream && !h->sums_valid) {
+            // nobody has summed this f yet (first step, or the caller rewrote it)
+            CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
+            h->sums_valid = true;
+            h->launches++;
+        }
         CU(launch_step(h->storage, h->plan, p, h->stream), "step kernel launch");
         h->cur ^= 1;
         h->parity ^= 1;
-        if (h->mesh.n_kin > 0) h->launches++;
+        if (h->mesh.n_kin > 0) h->launches += (stream && p.collide) ? 2 : 1;
     }
     return UFS_DVM_OK;
 }
@@ -201,6 +266,16 @@ int ufs_dvm_moments(ufs_dvm_t h, double* mom_dev) {
     if (h->sticky) return h->sticky;
     if (!mom_dev && h->mesh.n_kin > 0) return fail(h, UFS_DVM_EINVAL, "mom_dev is NULL");
     const StepParams p = make_params(h, 1.0);
+    if (h->plan.ring == 2 && h->mesh.n_kin > 0) {
+        if (!h->sums_valid) {
+            CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
+            h->sums_valid = true;
+            h->launches++;
+        }
+        CU(launch_moments_from_sums(p, h->d_sums[h->cur], mom_dev, h->stream), "moments kernel launch");
+        h->launches++;
+        return UFS_DVM_OK;
+    }
     CU(launch_moments(h->storage, p, h->f[h->cur], mom_dev, h->stream), "moments kernel launch");
     if (h->mesh.n_kin > 0) h->launches++;
     return UFS_DVM_OK;
@@ -226,12 +301,19 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) rc = UFS_DVM_ECUDA;
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
+        cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
     }
     delete h;
     return rc;
 }
 
 int ufs_dvm_current(ufs_dvm_t h) { return h ? h->cur : UFS_DVM_EINVAL; }
+
+int ufs_dvm_f_changed(ufs_dvm_t h) {
+    if (!h) return UFS_DVM_EINVAL;
+    h->sums_valid = false;
+    return UFS_DVM_OK;
+}
 
 int ufs_dvm_layout(ufs_dvm_t h, int64_t* n_kinetic, int64_t* cell_of_slab, int32_t* vel_of_slot) {
     if (!h) return UFS_DVM_EINVAL;
@@ -277,6 +359,7 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, doubl
     if (!f_host_in || !mom_dev_scratch || !mom_host) return fail(h, UFS_DVM_EINVAL, "NULL buffer");
     const size_t bytes = (size_t)h->mesh.n_kin * (size_t)h->mesh.vel.Nv * (h->storage == UFS_STORE_F32 ? 4 : 8);
     CU(cudaMemcpyAsync(h->f[h->cur], f_host_in, bytes, cudaMemcpyHostToDevice, h->stream), "copy f to the device");
+    h->sums_valid = false;
     int rc = ufs_dvm_step(h, dt, nsteps);
     if (rc) return rc;
     if ((rc = ufs_dvm_moments(h, mom_dev_scratch))) return rc;
@@ -298,7 +381,7 @@ int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int3
 
 const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
     if (!h) return "";
-    return h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
+    return h->plan.ring == 2 ? "k_stream" : h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
 }
 
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }

@@ -105,13 +105,13 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
                  : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
-// Blocks until the phase with the given parity has completed.  A watchdog turns a protocol bug into a
-// trap (reported as a CUDA error at the next sync) instead of a hung GPU.
+// Blocks until the phase with the given parity has completed (try_wait suspends the thread for a
+// hardware-defined time slice, so the loop is not a busy spin).  A watchdog turns a protocol bug into a trap
+// (reported as a CUDA error at the next sync) instead of a hung GPU.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 8000000000LL) __trap();  // ~4 s at 2 GHz
+        if (++spins > (1u << 26)) __trap();
     }
 }
 // global -> shared bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned); completion is

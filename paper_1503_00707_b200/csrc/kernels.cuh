@@ -36,11 +36,20 @@ struct StepParams {
     int32_t ring_stages;        // ring kernel: stages in the shared-memory ring
     int32_t l2_mode;            // ring kernel: L2 eviction hints on the bulk loads (0 none; see step_ring.cu)
     int32_t ticket_mode;        // ring kernel: how cells are handed to CTAs (see step_ring.cu)
+    // streaming step (step_stream.cu)
+    const double* sums_in;      // [n_kin][SUMS_STRIDE] velocity sums of f_in
+    double* sums_out;           // [n_kin][SUMS_STRIDE] velocity sums of f_out
+    const double* ghost_sums;   // [n_tables + n_fluid_ghosts][SUMS_STRIDE] the same sums of the ghost states
+    void* tabs;                 // [n_kin][tabn] storage type: Maxwellian factor tables + dt*nu of this step
+    int32_t n_tables;
 };
+
+constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used)
 
 struct StepLaunch {
     int32_t threads, smem_bytes, vec, fast;
-    int32_t ring;                  // 1: persistent TMA ring kernel (step_ring.cu), 0: one CTA per cell (kernels.cu)
+    int32_t ring;                  // 2: streaming step (step_stream.cu), 1: TMA ring kernel with an on-chip slab
+                                   // (step_ring.cu), 0: one CTA per cell (kernels.cu)
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
 };
 
@@ -60,6 +69,13 @@ int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** wh
 bool ring_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
 int ring_occupancy(int storage, const StepLaunch& plan);
 cudaError_t launch_ring(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
+
+// step_stream.cu: the streaming step (k_prep + k_stream), the sums of a freshly written f, moments from sums.
+bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
+int stream_tabn(const VelLayout& v);
+cudaError_t launch_stream(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
+cudaError_t launch_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
+cudaError_t launch_moments_from_sums(const StepParams& p, const double* sums, double* mom, cudaStream_t stream);
 
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);

@@ -35,6 +35,7 @@ def fill_initial_f_device(st: "B.DvmStepper", case: Case, chunk_slabs: int = 204
         a = n / (2 * np.pi * T) ** 1.5
         f = a * ez[:, kz] * ey[:, ky] * ex[:, kx]
         st.f[cur][s0:s0 + chunk_slabs].copy_(f.to(st.dtype))
+    B.ufs_dvm_f_changed(st.h)
 
 
 def window_leaves(case: Case, centre_leaf: int, rings: int, neighbours_of) -> np.ndarray:
