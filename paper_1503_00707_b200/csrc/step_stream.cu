@@ -24,7 +24,7 @@
 namespace ufs {
 namespace {
 
-enum { ST_SIMPLE = 0, ST_GATHER = 1, ST_STOP = 2 };
+enum { ST_RING = 0, ST_GATHER = 1, ST_STOP = 2 };
 constexpr int RED_SLOTS = 2;   // per-warp partial sums of the last two cells
 
 // ---------------------------------------------------------------- per-thread velocity constants
@@ -423,19 +423,62 @@ __device__ __forceinline__ void octant_from_ring(const StepParams& p, const Stre
 #pragma unroll
     for (int q = 0; q < PIECES; q++) {
         if (O + q > 0) mbar_wait(&s.full[slot], ph);
+        const int pe = PV * VEC;  // elements per piece
+        const int mask = s.info[slot].w;  // axes whose upwind face has four finer sources (reading G3); warp-uniform
+        T* const st = reinterpret_cast<T*>(s.ring + (size_t)slot * slot_bytes + (size_t)tid * 16);
+        if (mask) {
+            // The next three slots bring sources 1..3 of those axes (piece t = axis t).  They are added, in order,
+            // onto source 0 where it lies in this slot (each thread touches only its own 16 bytes), so the common
+            // path below needs no extra registers.
+            int sl = slot;
+            uint32_t sp = ph;
+#pragma unroll 1
+            for (int j = 1; j < 4; j++) {
+                if (++sl == NS) { sl = 0; sp ^= 1u; }
+                mbar_wait(&s.full[sl], sp);
+                if (active) {
+                    const T* se = reinterpret_cast<const T*>(s.ring + (size_t)sl * slot_bytes + (size_t)tid * 16);
+#pragma unroll 1
+                    for (int t = 0; t < 3; t++) {
+                        if ((mask >> t) & 1) {
+                            T v[VEC], x[VEC];
+                            lds16(se + t * pe, v);
+                            lds16(st + (t + 1) * pe, x);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) x[i] += v[i];
+                            sts16(st + (t + 1) * pe, x);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s.empty[sl]);
+            }
+        }
+        T own[VEC], X[VEC], Y[VEC], Z[VEC];
         if (active) {
-            const T* st = reinterpret_cast<const T*>(s.ring + (size_t)slot * slot_bytes + (size_t)tid * 16);
-            const int pe = PV * VEC;  // elements per piece
-            T own[VEC], X[VEC], Y[VEC], Z[VEC];
             lds16(st, own);
             lds16(st + pe, X);
             lds16(st + 2 * pe, Y);
             lds16(st + 3 * pe, Z);
+            if (mask) {  // each of the four sources weighs 1/4
+#pragma unroll
+                for (int i = 0; i < VEC; i++) {
+                    if (mask & 1) X[i] *= T(0.25);
+                    if (mask & 2) Y[i] *= T(0.25);
+                    if (mask & 4) Z[i] *= T(0.25);
+                }
+            }
             finish_vec<T, O, PIECES>(p, cc, q, pos[q], nhp, own, X, Y, Z, gout + O * CH + q * pe, acc);
         }
+        // this slot was written with ordinary stores: order them before the bulk copy that refills it
+        if (mask) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(&s.empty[slot]);
         if (++slot == NS) { slot = 0; ph ^= 1u; }
+        if (mask) {  // step over the three slots consumed above
+#pragma unroll 1
+            for (int j = 1; j < 4; j++) if (++slot == NS) { slot = 0; ph ^= 1u; }
+        }
     }
 }
 
@@ -502,12 +545,16 @@ __global__ void __launch_bounds__((NCW + 2) * 32, 1) k_stream(const StepParams p
                 break;
             }
             const int level = __shfl_sync(0xffffffffu, rec, 24), flags = __shfl_sync(0xffffffffu, rec, 25);
-            const bool simple = (flags & CELL_SIMPLE) != 0;
+            const bool ringable = (flags & CELL_NOFLUID) != 0;
+            // bit d: direction d has four (finer) sources instead of one
+            int four = 0;
+#pragma unroll
+            for (int d = 0; d < 6; d++) four |= (__shfl_sync(0xffffffffu, rec, d * 4 + 1) >= 0 ? 1 : 0) << d;
             // the first stage of a cell also carries its factor table (behind the four pieces of the slot)
             void* tab_dst = s.ring + (size_t)slot * slot_bytes + stage_bytes;
             const T* tab_src = reinterpret_cast<const T*>(p.tabs) + (int64_t)cur * tabn;
             const uint32_t extra = p.collide ? tab_bytes : 0u;
-            if (simple) {
+            if (ringable) {
                 // lane (o,t): stream t of octant o -- t = 0 own chunk, t = 1..3 the upwind chunk on axis t-1
                 const int a = t_l > 0 ? t_l - 1 : 0;
                 const int dir = 2 * a + (1 - ((o_l >> a) & 1));
@@ -520,12 +567,18 @@ __global__ void __launch_bounds__((NCW + 2) * 32, 1) k_stream(const StepParams p
                 for (int o = 0; o < 8; o++) {
                     // the next ticket is drawn late, so that the cells in flight stay consecutive in slab order
                     if (o == 7) nxt_raw = fetch_async();
+                    // axes whose upwind face of this octant has four finer sources: sources 1..3 follow in three
+                    // more slots (piece t = axis t)
+                    int mask = 0;
+#pragma unroll
+                    for (int b = 0; b < 3; b++) mask |= ((four >> (2 * b + (1 - ((o >> b) & 1)))) & 1) << b;
+                    const int xdir = lane < 3 ? 2 * lane + (1 - ((o >> lane) & 1)) : 0;
 #pragma unroll
                     for (int q = 0; q < PIECES; q++) {
                         const bool first = (o + q) == 0;
                         mbar_wait(&s.empty[slot], ph ^ 1u);
                         if (lane == 0) {
-                            s.info[slot] = make_int4(cur, level, ST_SIMPLE, o * PIECES + q);
+                            s.info[slot] = make_int4(cur, level, ST_RING, mask);
                             mbar_arrive_expect_tx(&s.full[slot], stage_bytes + (first ? extra : 0u));
                             if (first && extra) bulk_g2s(tab_dst, tab_src, tab_bytes, &s.full[slot]);
                         }
@@ -535,6 +588,27 @@ __global__ void __launch_bounds__((NCW + 2) * 32, 1) k_stream(const StepParams p
                             bulk_g2s(dst, ptr + (size_t)q * PV * VEC, piece_bytes, &s.full[slot]);
                         }
                         advance();
+                        if (mask) {
+#pragma unroll 1
+                            for (int j = 1; j < 4; j++) {
+                                const int xcode = __shfl_sync(0xffffffffu, rec, xdir * 4 + j);
+                                mbar_wait(&s.empty[slot], ph ^ 1u);
+                                if (lane == 0) {
+                                    s.info[slot] = make_int4(cur, level, ST_RING, mask);
+                                    mbar_arrive_expect_tx(&s.full[slot], (uint32_t)__popc(mask) * piece_bytes);
+                                }
+                                __syncwarp();
+                                if (lane < 3 && ((mask >> lane) & 1)) {
+                                    const int xkind = xcode >> SRC_SHIFT;
+                                    const int64_t xidx = xcode & SRC_INDEX_MASK;
+                                    const T* xptr = (xkind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + xidx * p.Nv
+                                                    + (int64_t)(xkind == SRC_MIRROR ? (o ^ (1 << lane)) : o) * CH;
+                                    void* dst = s.ring + (size_t)slot * slot_bytes + (size_t)lane * piece_bytes;
+                                    bulk_g2s(dst, xptr + (size_t)q * PV * VEC, piece_bytes, &s.full[slot]);
+                                }
+                                advance();
+                            }
+                        }
                     }
                 }
             } else {
@@ -624,7 +698,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, 1) k_stream(const StepParams p
         double acc[35];
 #pragma unroll
         for (int i = 0; i < 35; i++) acc[i] = 0.0;
-        if (inf.z == ST_SIMPLE) {
+        if (inf.z == ST_RING) {
 #define UFS_OCT(O) octant_from_ring<T, O, PIECES>(p, s, cc, pos, nhp, PV, CH, active, tid, lane, gout, acc, slot, ph, NS, slot_bytes);
             UFS_OCT(0) UFS_OCT(1) UFS_OCT(2) UFS_OCT(3) UFS_OCT(4) UFS_OCT(5) UFS_OCT(6) UFS_OCT(7)
 #undef UFS_OCT
@@ -734,8 +808,8 @@ bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan
     const size_t stage = (size_t)4 * (chv / pieces) * 16;
     const int tabn = tabn_of(v.nh);
     int ns = 16 * pieces;  // at most two cells deep
-    while (ns >= 3 && stream_smem_bytes(elem, ns, stage, ncw, tabn) > SMEM_PER_CTA_MAX) ns--;
-    if (ns < 3) return false;
+    while (ns >= 4 && stream_smem_bytes(elem, ns, stage, ncw, tabn) > SMEM_PER_CTA_MAX) ns--;
+    if (ns < 4) return false;  // a 2:1 face needs four slots in flight at once
     plan->ring = 2;
     plan->ncw = ncw;
     plan->pieces = pieces;
