@@ -99,6 +99,13 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.ghost_sums = h->d_ghost_sums;
     p.tabs = h->d_tabs;
     p.n_tables = h->mesh.n_tables;
+    if (v.fast) {
+        for (int r = 0; r < v.nh[0] && r < 16; r++) {
+            const double x = v.xi[0][v.nh[0] + r];
+            p.xpow[0][r] = x; p.xpow[1][r] = x * x; p.xpow[2][r] = x * x * x;
+            p.xf[r] = (float)x;
+        }
+    }
     return p;
 }
 
@@ -199,7 +206,10 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
         CU(cudaGetDevice(&dev), "get device");
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
         StepLaunch cand{};
-        if (!want_ring && stream_plan(h->storage, v, sms, &cand)) {
+        const bool want_vec = force && std::strcmp(force, "stream") == 0;   // the one-vector-per-thread variant
+        if (!want_ring && !want_vec && rows_plan(h->storage, v, sms, &cand)) {
+            h->plan = cand;
+        } else if (!want_ring && stream_plan(h->storage, v, sms, &cand)) {
             h->plan = cand;
         } else if (ring_plan(h->storage, v, sms, &cand)) {
             const int occ = ring_occupancy(h->storage, cand);
@@ -209,7 +219,7 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
             }
         }
     }
-    if (h->plan.ring == 2 && m.n_kin > 0) {
+    if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
         const size_t sums_bytes = (size_t)m.n_kin * SUMS_STRIDE * sizeof(double);
         for (int b = 0; b < 2; b++) CU(cudaMalloc(reinterpret_cast<void**>(&h->d_sums[b]), sums_bytes), "allocate velocity sums");
@@ -243,7 +253,7 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!(dt > 0) || nsteps < 0) return fail(h, UFS_DVM_EINVAL, "dt must be positive and nsteps >= 0");
-    const bool stream = h->plan.ring == 2 && h->mesh.n_kin > 0;
+    const bool stream = h->plan.ring >= 2 && h->mesh.n_kin > 0;
     for (int s = 0; s < nsteps; s++) {
         const StepParams p = make_params(h, dt);
         if (stream && !h->sums_valid) {
@@ -266,7 +276,7 @@ int ufs_dvm_moments(ufs_dvm_t h, double* mom_dev) {
     if (h->sticky) return h->sticky;
     if (!mom_dev && h->mesh.n_kin > 0) return fail(h, UFS_DVM_EINVAL, "mom_dev is NULL");
     const StepParams p = make_params(h, 1.0);
-    if (h->plan.ring == 2 && h->mesh.n_kin > 0) {
+    if (h->plan.ring >= 2 && h->mesh.n_kin > 0) {
         if (!h->sums_valid) {
             CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
             h->sums_valid = true;
@@ -381,7 +391,7 @@ int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int3
 
 const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
     if (!h) return "";
-    return h->plan.ring == 2 ? "k_stream" : h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
+    return h->plan.ring == 3 ? "k_rows" : h->plan.ring == 2 ? "k_stream" : h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
 }
 
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }

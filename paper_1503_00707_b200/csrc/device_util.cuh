@@ -108,12 +108,30 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 // Blocks until the phase with the given parity has completed (try_wait suspends the thread for a
 // hardware-defined time slice, so the loop is not a busy spin).  A watchdog turns a protocol bug into a trap
 // (reported as a CUDA error at the next sync) instead of a hung GPU.
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+#ifdef UFS_DEBUG_WAIT
+static __device__ int g_dbg[8];
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int code = 0) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        ++spins;
+        if ((spins & 1023u) == 0 && *((volatile int*)&g_dbg[0]) != 0) return;
+        if (spins > (1u << 20)) {
+            if (atomicCAS(&g_dbg[0], 0, code + 1000) == 0) {
+                g_dbg[1] = blockIdx.x; g_dbg[2] = threadIdx.x >> 5; g_dbg[3] = (int)parity;
+                g_dbg[4] = (int)(smem_u32(bar));
+            }
+            return;
+        }
+    }
+}
+#else
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int = 0) {
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
         if (++spins > (1u << 26)) __trap();
     }
 }
+#endif
 // global -> shared bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned); completion is
 // signalled on `bar` as a transaction count
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {

@@ -42,13 +42,17 @@ struct StepParams {
     const double* ghost_sums;   // [n_tables + n_fluid_ghosts][SUMS_STRIDE] the same sums of the ghost states
     void* tabs;                 // [n_kin][tabn] storage type: Maxwellian factor tables + dt*nu of this step
     int32_t n_tables;
+    // row kernel (step_rows.cu): |xi_x| of the x ranks and its powers (uniform operands, constant bank)
+    double xpow[3][16];         // [r-1][rank] = |xi_x|^r, r = 1..3
+    float xf[16];               // |xi_x| in fp32
 };
 
 constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used)
 
 struct StepLaunch {
     int32_t threads, smem_bytes, vec, fast;
-    int32_t ring;                  // 2: streaming step (step_stream.cu), 1: TMA ring kernel with an on-chip slab
+    int32_t ring;                  // 3: streaming step, one row per thread (step_rows.cu), 2: streaming step, one
+                                   // vector per thread (step_stream.cu), 1: TMA ring kernel with an on-chip slab
                                    // (step_ring.cu), 0: one CTA per cell (kernels.cu)
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
 };
@@ -74,6 +78,10 @@ cudaError_t launch_ring(int storage, const StepLaunch& plan, const StepParams& p
 bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
 int stream_tabn(const VelLayout& v);
 cudaError_t launch_stream(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
+cudaError_t launch_prep(int storage, const StepParams& p, cudaStream_t stream);   // k_prep alone
+// step_rows.cu: the same step with one velocity row per thread
+bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
+cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 cudaError_t launch_moments_from_sums(const StepParams& p, const double* sums, double* mom, cudaStream_t stream);
 

@@ -20,6 +20,7 @@
 
 #include "device_util.cuh"
 #include "kernels.cuh"
+#include "stream_common.cuh"
 
 namespace ufs {
 namespace {
@@ -56,10 +57,6 @@ __device__ __forceinline__ Pos<T> pos_of(const StepParams& p, int v) {
     return c;
 }
 
-// ---------------------------------------------------------------- the cell sums (SUMS_STRIDE doubles per cell)
-// [0..4] H,  [5 + (2a+s)*5 + k] G[a][s][k];  s = 1: xi_a > 0.
-__device__ __forceinline__ constexpr int g_index(int a, int s, int k) { return 5 + (2 * a + s) * 5 + k; }
-
 // a2': fold one vector of the new f (octant O) into the thread's 35 partial sums.  Four sums along the x run
 // (1, |xi_x|, xi_x^2, |xi_x|^3 weights), then the y/z weights and the signs once per vector.
 template <typename T, int O>
@@ -95,80 +92,6 @@ __device__ __forceinline__ void add_sums(const T (&f)[V16<T>::N], const Pos<T>& 
     }
 }
 
-// Warp-level sum of the 35 partials, stored to dst[0..35].  Butterfly with halving: at each of the five exchange
-// steps a lane keeps one half of its values and hands the other half to its partner, so 36 -> 18 -> 9 -> 5 -> 3 -> 2
-// values per lane and 37 exchanges in all (a plain shuffle reduction of 35 values takes 175).
-template <int N, int OFF>
-__device__ __forceinline__ void halve(double (&v)[36], int lane) {
-    constexpr int H = (N + 1) / 2;
-    const bool up = (lane & OFF) != 0;
-#pragma unroll
-    for (int i = 0; i < H; i++) {
-        const double a = v[i], b = (i + H < N) ? v[i + H] : 0.0;
-        const double recv = __shfl_xor_sync(0xffffffffu, up ? a : b, OFF);
-        v[i] = (up ? b : a) + recv;
-    }
-}
-__device__ __forceinline__ void warp_store_sums(const double (&acc)[35], double* dst, int lane) {
-    double v[36];
-#pragma unroll
-    for (int i = 0; i < 35; i++) v[i] = acc[i];
-    v[35] = 0.0;
-    halve<36, 16>(v, lane);
-    halve<18, 8>(v, lane);
-    halve<9, 4>(v, lane);
-    halve<5, 2>(v, lane);
-    halve<3, 1>(v, lane);
-    // lane holds v[t], t = 0, 1: entry t + 2 b0 + 3 b1 + 5 b2 + 9 b3 + 18 b4 of the sums (if every partial index is real)
-    const int b0 = lane & 1, b1 = (lane >> 1) & 1, b2 = (lane >> 2) & 1, b3 = (lane >> 3) & 1, b4 = (lane >> 4) & 1;
-#pragma unroll
-    for (int t = 0; t < 2; t++) {
-        const int j4 = t + 2 * b0, j3 = j4 + 3 * b1, j2 = j3 + 5 * b2, j1 = j2 + 9 * b3, j0 = j1 + 18 * b4;
-        if (j4 < 3 && j3 < 5 && j2 < 9 && j1 < 18 && j0 < 36) dst[j0] = v[t];
-    }
-}
-
-// ---------------------------------------------------------------- gather path (cells that are not "simple")
-// value of the upwind source on axis a for octant o: one chunk, or 4 finer neighbours each weighted 1/4
-// (reading G3), or the pointwise Maxwellian of a fluid leaf's frozen moments
-template <typename T>
-__device__ __forceinline__ void gather_axis(const StepParams& p, const int* __restrict__ rec, const T* fin, int a, int o,
-                                            int CH, int e, const Pos<T>& c, T (&out)[V16<T>::N]) {
-    constexpr int VEC = V16<T>::N;
-    const int s = (o >> a) & 1;
-    const int dir = 2 * a + (1 - s);  // xi_a > 0: data comes from the low side
-    const int n = __ldg(rec + dir * 4 + 1) >= 0 ? 4 : 1;
-    T acc[VEC];
-#pragma unroll
-    for (int i = 0; i < VEC; i++) acc[i] = T(0);
-    for (int k = 0; k < n; k++) {
-        const int code = __ldg(rec + dir * 4 + k);
-        const int kind = code >> SRC_SHIFT;
-        const int64_t idx = code & SRC_INDEX_MASK;
-        if (kind == SRC_FLUID) {
-            const FluidGhost* g = p.fluid + idx;
-            const int kz = ((o >> 2) & 1) ? p.nh[2] + c.rz : p.nh[2] - 1 - c.rz;
-            const int ky = ((o >> 1) & 1) ? p.nh[1] + c.ry : p.nh[1] - 1 - c.ry;
-            const double b = g->amp * g->g[2][kz] * g->g[1][ky];
-#pragma unroll
-            for (int i = 0; i < VEC; i++) {
-                const int kx = (o & 1) ? p.nh[0] + c.rx + i : p.nh[0] - 1 - c.rx - i;
-                acc[i] += (T)(b * g->g[0][kx]);
-            }
-        } else {
-            const T* base = (kind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + idx * p.Nv
-                            + (int64_t)(kind == SRC_MIRROR ? (o ^ (1 << a)) : o) * CH;
-            T v[VEC];
-            ldg16(base + e, v);
-#pragma unroll
-            for (int i = 0; i < VEC; i++) acc[i] += v[i];
-        }
-    }
-    const T wgt = (n == 4) ? T(0.25) : T(1);
-#pragma unroll
-    for (int i = 0; i < VEC; i++) out[i] = acc[i] * wgt;
-}
-
 // ---------------------------------------------------------------- k_prep: rho* and the discrete Maxwellian (a2, a3)
 // 1/x to about one ulp: hardware seed (20 bits) + two Newton steps
 __device__ __forceinline__ double frcp(double x) {
@@ -182,15 +105,6 @@ __device__ __forceinline__ double frcp(double x) {
 template <typename T> struct SeriesTol;   // residual below which one more (series) update ends the solve
 template <> struct SeriesTol<double> { static constexpr double value = 1e-7; };   // error after it ~1e-14
 template <> struct SeriesTol<float> { static constexpr double value = 1e-4; };    // ~1e-8 << fp32 storage rounding
-
-// Table layout of one cell (TABN elements of T): [axis][sign][nhp] factors by rank of |xi|
-// (axis 2 carries the amplitude), then dt*nu.
-__host__ __device__ inline int nhp_of(const int32_t nh[3]) {
-    int m = nh[0] > nh[1] ? nh[0] : nh[1];
-    m = m > nh[2] ? m : nh[2];
-    return (m + 3) & ~3;
-}
-__host__ __device__ inline int tabn_of(const int32_t nh[3]) { return 6 * nhp_of(nh) + 4; }
 
 // Solve  w sum_i m(xi_i) exp(alpha . m(xi_i)) = rho with one warp.  exp(alpha.m) = A gx gy gz,
 // g_b[k] = exp(alpha_b xi_k + alpha_4 xi_k^2).  With the 1-D power sums P_b^r = sum_k xi_k^r g_b[k] the five
@@ -493,9 +407,9 @@ __device__ __forceinline__ void octant_from_gather(const StepParams& p, const Ce
         const int e = q * pe + tid * VEC;
         T own[VEC], X[VEC], Y[VEC], Z[VEC];
         ldg16(own_base + O * CH + q * pe, own);
-        gather_axis<T>(p, rec, fin, 0, O, CH, e, pos[q], X);
-        gather_axis<T>(p, rec, fin, 1, O, CH, e, pos[q], Y);
-        gather_axis<T>(p, rec, fin, 2, O, CH, e, pos[q], Z);
+        gather_axis<T>(p, rec, fin, 0, O, CH, e, pos[q].rx, pos[q].ry, pos[q].rz, X);
+        gather_axis<T>(p, rec, fin, 1, O, CH, e, pos[q].rx, pos[q].ry, pos[q].rz, Y);
+        gather_axis<T>(p, rec, fin, 2, O, CH, e, pos[q].rx, pos[q].ry, pos[q].rz, Z);
         finish_vec<T, O, PIECES>(p, cc, q, pos[q], nhp, own, X, Y, Z, gout + O * CH + q * pe, acc);
     }
 }
@@ -820,6 +734,14 @@ bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan
     plan->fast = 1;
     plan->grid = sm_count;
     return true;
+}
+
+cudaError_t launch_prep(int storage, const StepParams& p, cudaStream_t st) {
+    if (p.n_kin == 0 || !p.collide) return cudaSuccess;
+    const int wpb = 8;
+    if (storage == UFS_STORE_F32) k_prep<float><<<(p.n_kin + wpb - 1) / wpb, wpb * 32, 0, st>>>(p);
+    else k_prep<double><<<(p.n_kin + wpb - 1) / wpb, wpb * 32, 0, st>>>(p);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_stream(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
