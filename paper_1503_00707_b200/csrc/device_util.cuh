@@ -143,4 +143,55 @@ __device__ __forceinline__ void bulk_g2s_hint(void* dst_smem, const void* src, u
                  ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
 
+// ---- the same primitives on 32-bit shared-space addresses (no generic-pointer conversion, one register) ----
+__device__ __forceinline__ void smbar_arrive(uint32_t bar) {
+    asm volatile("{ .reg .b64 t; mbarrier.arrive.shared::cta.b64 t, [%0]; }" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void smbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("{ .reg .b64 t; mbarrier.arrive.expect_tx.shared::cta.b64 t, [%0], %1; }" ::"r"(bar), "r"(bytes) : "memory");
+}
+// try_wait with a suspend-time hint: the thread sleeps in hardware until the phase completes or the hint elapses
+__device__ __forceinline__ bool smbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void smbar_wait(uint32_t bar, uint32_t parity) {
+#ifdef UFS_DEBUG_WAIT
+    uint32_t spins = 0;
+    while (!smbar_try_wait(bar, parity)) {
+        if (++spins > (1u << 9)) __trap();
+    }
+#else
+    while (!smbar_try_wait(bar, parity)) {}
+#endif
+}
+__device__ __forceinline__ void sbulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void slds16(uint32_t a, float (&r)[4]) {
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]) : "r"(a));
+}
+__device__ __forceinline__ void slds16(uint32_t a, double (&r)[2]) {
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(r[0]), "=d"(r[1]) : "r"(a));
+}
+__device__ __forceinline__ void ssts16(uint32_t a, const float (&r)[4]) {
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]) : "memory");
+}
+__device__ __forceinline__ void ssts16(uint32_t a, const double (&r)[2]) {
+    asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(a), "d"(r[0]), "d"(r[1]) : "memory");
+}
+__device__ __forceinline__ float slds(uint32_t a, float) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ double slds(uint32_t a, double) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ int slds_i32(uint32_t a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ int slds_i32_volatile(uint32_t a) { int v; asm volatile("ld.volatile.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ void ssts_i32_volatile(uint32_t a, int v) { asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+
+// pull `bytes` (multiple of 16) at a global address into L2 without a destination (TMA prefetch)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+
 }  // namespace ufs

@@ -16,6 +16,7 @@
 // of k_prep) travels in a small ring of cell headers.  The warp that finishes a cell last adds up the per-warp
 // partial sums and writes the cell's 35 velocity sums for the next step.
 #include <cmath>
+#include <cstdlib>
 
 #include "device_util.cuh"
 #include "kernels.cuh"
@@ -26,41 +27,44 @@ namespace {
 
 enum { CK_RING = 0, CK_GATHER = 1, CK_STOP = 2 };
 constexpr int CELL_SLOTS = 3;
-constexpr int HDR_INTS = 16;  // cell, level, kind, -, masks[8], -
+constexpr int HDR_REC = 16;   // header ints: cell, level, kind, mbits, masks, -..., then the 32 words of the cell record
+constexpr int HDR_INTS = 48;
 
+// Shared-memory map of a CTA (byte offsets from the start of dynamic shared memory).
 struct RowsSmem {
-    unsigned char* ring;   // [NS][slot_bytes]: 4 pieces
-    unsigned char* cells;  // [CELL_SLOTS][cell_bytes]: HDR_INTS ints, then the factor table
-    double* red;           // [CELL_SLOTS][NW][SUMS_STRIDE]
-    double2* ayz;          // [NR] |xi_y|, |xi_z| of each row
-    uint64_t* full;        // [NS]
-    uint64_t* empty;       // [NS]
-    uint64_t* cfull;       // [CELL_SLOTS]
-    uint64_t* cempty;      // [CELL_SLOTS]
-    int* cnt;              // [CELL_SLOTS] warps that have delivered their partial sums
+    uint32_t ring;    // [NS][slot_bytes]: 4 pieces
+    uint32_t cells;   // [CELL_SLOTS][cell_bytes]: HDR_INTS ints, then the factor table
+    uint32_t red;     // [CELL_SLOTS][NW][SUMS_STRIDE] doubles
+    uint32_t ayz;     // [NR] double2: |xi_y|, |xi_z| of each row
+    uint32_t full;    // [NS] mbarriers
+    uint32_t empty;   // [NS]
+    uint32_t cfull;   // [CELL_SLOTS]
+    uint32_t cempty;  // [CELL_SLOTS]
+    uint32_t cnt;     // [CELL_SLOTS] ints: warps that have delivered their partial sums
+    uint32_t issued;  // int: ring slots armed by the producer so far
+    uint32_t total;
 };
 __host__ __device__ inline size_t rows_cell_bytes(size_t elem, int tabn) {
     return ((size_t)HDR_INTS * 4 + (size_t)tabn * elem + 127) & ~(size_t)127;
 }
-__host__ __device__ inline size_t rows_smem_bytes(size_t elem, int ns, size_t slot_bytes, int nw, int tabn, int nr) {
-    size_t b = (size_t)ns * slot_bytes + CELL_SLOTS * rows_cell_bytes(elem, tabn);
-    b += (size_t)CELL_SLOTS * nw * SUMS_STRIDE * 8 + (size_t)nr * 16;
-    b += (size_t)ns * 16 + CELL_SLOTS * 16 + CELL_SLOTS * 4 + 16;
-    return (b + 127) & ~(size_t)127;
-}
-__device__ __forceinline__ RowsSmem rows_carve(unsigned char* base, size_t elem, int ns, size_t slot_bytes, int nw, int tabn, int nr) {
+__host__ __device__ inline RowsSmem rows_map(size_t elem, int ns, size_t slot_bytes, int nw, int tabn, int nr) {
     RowsSmem s;
     size_t off = 0;
-    s.ring = base; off += (size_t)ns * slot_bytes;
-    s.cells = base + off; off += CELL_SLOTS * rows_cell_bytes(elem, tabn);
-    s.red = reinterpret_cast<double*>(base + off); off += (size_t)CELL_SLOTS * nw * SUMS_STRIDE * 8;
-    s.ayz = reinterpret_cast<double2*>(base + off); off += (size_t)nr * 16;
-    s.full = reinterpret_cast<uint64_t*>(base + off); off += (size_t)ns * 8;
-    s.empty = reinterpret_cast<uint64_t*>(base + off); off += (size_t)ns * 8;
-    s.cfull = reinterpret_cast<uint64_t*>(base + off); off += CELL_SLOTS * 8;
-    s.cempty = reinterpret_cast<uint64_t*>(base + off); off += CELL_SLOTS * 8;
-    s.cnt = reinterpret_cast<int*>(base + off);
+    s.ring = (uint32_t)off; off += (size_t)ns * slot_bytes;
+    s.cells = (uint32_t)off; off += CELL_SLOTS * rows_cell_bytes(elem, tabn);
+    s.red = (uint32_t)off; off += (size_t)CELL_SLOTS * nw * SUMS_STRIDE * 8;
+    s.ayz = (uint32_t)off; off += (size_t)nr * 16;
+    s.full = (uint32_t)off; off += (size_t)ns * 8;
+    s.empty = (uint32_t)off; off += (size_t)ns * 8;
+    s.cfull = (uint32_t)off; off += CELL_SLOTS * 8;
+    s.cempty = (uint32_t)off; off += CELL_SLOTS * 8;
+    s.cnt = (uint32_t)off; off += CELL_SLOTS * 4;
+    s.issued = (uint32_t)off; off += 8;
+    s.total = (uint32_t)((off + 127) & ~(size_t)127);
     return s;
+}
+__host__ __device__ inline size_t rows_smem_bytes(size_t elem, int ns, size_t slot_bytes, int nw, int tabn, int nr) {
+    return rows_map(elem, ns, slot_bytes, nw, tabn, nr).total;
 }
 
 // fold the four x sums of one row of octant O into the thread's 35 partial sums (layout: stream_common.cuh)
@@ -111,88 +115,102 @@ struct RowCtx {
     T base[NQ], cy[NQ], cz[NQ];  // (1 - dt nu) (1 - dt/h (|xi_y| + |xi_z|)), (1 - dt nu) dt/h |xi_y|, ... |xi_z|
     T sx;                        // (1 - dt nu) dt/h: times |xi_x,k| it is the x coefficient
     T omega;                     // dt nu
-    double ay[NQ], az[NQ];
-    int ry[NQ], rz[NQ];
 };
 
-// One row from four shared-memory streams: transport + relaxation + store + the four x sums (a1, a4, a2').
+// One row of values already in registers: transport + relaxation + store + the four x sums (a1, a4, a2').
 template <typename T, int NHX, int NQ>
+__device__ __forceinline__ void row_finish(const StepParams& p, const RowCtx<T, NQ>& rc, int q, T wb, int j, const T (&own)[V16<T>::N],
+                                           const T (&X)[V16<T>::N], const T (&Y)[V16<T>::N], const T (&Z)[V16<T>::N],
+                                           const T* gxrow, T* gdst, double& s0, double& s1, double& s2, double& s3) {
+    constexpr int VEC = V16<T>::N;
+    T out[VEC];
+#pragma unroll
+    for (int i = 0; i < VEC; i++) {
+        const T cx = rc.sx * x_of<T>(p, j * VEC + i);
+        out[i] = rc.base[q] * own[i] + cx * (X[i] - own[i]) + rc.cy[q] * Y[i] + rc.cz[q] * Z[i];
+    }
+    if (p.collide) {
+        T gx[VEC];
+        lds16(gxrow + j * VEC, gx);
+#pragma unroll
+        for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+    }
+    stg16_cs(gdst + j * VEC, out);
+#pragma unroll
+    for (int i = 0; i < VEC; i++) {
+        const int k = j * VEC + i;
+        const double d = (double)out[i];
+        s0 += d;
+        s1 = fma(p.xpow[0][k], d, s1);
+        s2 = fma(p.xpow[1][k], d, s2);
+        s3 = fma(p.xpow[2][k], d, s3);
+    }
+}
+
+// One row from the four streams of a ring slot.  EARLY: the whole row is read into registers first and the slot is
+// handed back to the producer before the arithmetic (the ring then holds data in flight, not data in use).
+template <typename T, int NHX, int NQ, bool EARLY>
 __device__ __forceinline__ void row_from_ring(const StepParams& p, const RowCtx<T, NQ>& rc, int q, T wb, const T* st, int pe,
-                                              const T* gxrow, T* gdst, double& s0, double& s1, double& s2, double& s3) {
+                                              const T* gxrow, T* gdst, bool active, int lane, uint32_t empty_bar, double& s0,
+                                              double& s1, double& s2, double& s3) {
     constexpr int VEC = V16<T>::N, RV = NHX / VEC;
+    if (EARLY) {
+        T own[RV][VEC], X[RV][VEC], Y[RV][VEC], Z[RV][VEC];
+        if (active) {
 #pragma unroll
-    for (int j = 0; j < RV; j++) {
-        T own[VEC], X[VEC], Y[VEC], Z[VEC], out[VEC];
-        lds16(st + j * VEC, own);
-        lds16(st + pe + j * VEC, X);
-        lds16(st + 2 * pe + j * VEC, Y);
-        lds16(st + 3 * pe + j * VEC, Z);
-#pragma unroll
-        for (int i = 0; i < VEC; i++) {
-            const int k = j * VEC + i;
-            const T cx = rc.sx * x_of<T>(p, k);
-            out[i] = rc.base[q] * own[i] + cx * (X[i] - own[i]) + rc.cy[q] * Y[i] + rc.cz[q] * Z[i];
+            for (int j = 0; j < RV; j++) {
+                lds16(st + j * VEC, own[j]);
+                lds16(st + pe + j * VEC, X[j]);
+                lds16(st + 2 * pe + j * VEC, Y[j]);
+                lds16(st + 3 * pe + j * VEC, Z[j]);
+            }
         }
-        if (p.collide) {
-            T gx[VEC];
-            lds16(gxrow + j * VEC, gx);
+        __syncwarp();
+        if (lane == 0) smbar_arrive(empty_bar);
+        if (active) {
 #pragma unroll
-            for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+            for (int j = 0; j < RV; j++) row_finish<T, NHX, NQ>(p, rc, q, wb, j, own[j], X[j], Y[j], Z[j], gxrow, gdst, s0, s1, s2, s3);
         }
-        stg16_cs(gdst + j * VEC, out);
+    } else {
+        if (active) {
 #pragma unroll
-        for (int i = 0; i < VEC; i++) {
-            const int k = j * VEC + i;
-            const double d = (double)out[i];
-            s0 += d;
-            s1 = fma(p.xpow[0][k], d, s1);
-            s2 = fma(p.xpow[1][k], d, s2);
-            s3 = fma(p.xpow[2][k], d, s3);
+            for (int j = 0; j < RV; j++) {
+                T own[VEC], X[VEC], Y[VEC], Z[VEC];
+                lds16(st + j * VEC, own);
+                lds16(st + pe + j * VEC, X);
+                lds16(st + 2 * pe + j * VEC, Y);
+                lds16(st + 3 * pe + j * VEC, Z);
+                row_finish<T, NHX, NQ>(p, rc, q, wb, j, own, X, Y, Z, gxrow, gdst, s0, s1, s2, s3);
+            }
         }
+        __syncwarp();
+        if (lane == 0) smbar_arrive(empty_bar);
     }
 }
 
 // The same row for a cell with a kinetic/fluid face: sources gathered with plain loads.
 template <typename T, int NHX, int NQ>
 __device__ __forceinline__ void row_from_gather(const StepParams& p, const RowCtx<T, NQ>& rc, int q, T wb, int o, int CH, int row,
-                                                const int* rec, const T* fin, int cell, const T* gxrow, T* gdst,
+                                                int ry, int rz, const int* rec, const T* fin, int cell, const T* gxrow, T* gdst,
                                                 double& s0, double& s1, double& s2, double& s3) {
     constexpr int VEC = V16<T>::N, RV = NHX / VEC;
     const T* own_base = fin + (int64_t)cell * p.Nv + (int64_t)o * CH + (int64_t)row * NHX;
 #pragma unroll 1
     for (int j = 0; j < RV; j++) {
-        T own[VEC], X[VEC], Y[VEC], Z[VEC], out[VEC];
+        T own[VEC], X[VEC], Y[VEC], Z[VEC];
         const int e = row * NHX + j * VEC;
         ldg16(own_base + j * VEC, own);
-        gather_axis<T>(p, rec, fin, 0, o, CH, e, j * VEC, rc.ry[q], rc.rz[q], X);
-        gather_axis<T>(p, rec, fin, 1, o, CH, e, j * VEC, rc.ry[q], rc.rz[q], Y);
-        gather_axis<T>(p, rec, fin, 2, o, CH, e, j * VEC, rc.ry[q], rc.rz[q], Z);
-#pragma unroll
-        for (int i = 0; i < VEC; i++) {
-            const T cx = rc.sx * x_of<T>(p, j * VEC + i);
-            out[i] = rc.base[q] * own[i] + cx * (X[i] - own[i]) + rc.cy[q] * Y[i] + rc.cz[q] * Z[i];
-        }
-        if (p.collide) {
-            T gx[VEC];
-            lds16(gxrow + j * VEC, gx);
-#pragma unroll
-            for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
-        }
-        stg16_cs(gdst + j * VEC, out);
-#pragma unroll
-        for (int i = 0; i < VEC; i++) {
-            const double d = (double)out[i];
-            s0 += d;
-            s1 = fma(p.xpow[0][j * VEC + i], d, s1);
-            s2 = fma(p.xpow[1][j * VEC + i], d, s2);
-            s3 = fma(p.xpow[2][j * VEC + i], d, s3);
-        }
+        gather_axis<T>(p, rec, fin, 0, o, CH, e, j * VEC, ry, rz, X);
+        gather_axis<T>(p, rec, fin, 1, o, CH, e, j * VEC, ry, rz, Y);
+        gather_axis<T>(p, rec, fin, 2, o, CH, e, j * VEC, ry, rz, Z);
+        row_finish<T, NHX, NQ>(p, rc, q, wb, j, own, X, Y, Z, gxrow, gdst, s0, s1, s2, s3);
     }
 }
 
-template <typename T, int NHX, int GW, int NG, int NQ>
+template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY>
 __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams p) {
     constexpr int VEC = V16<T>::N, RV = NHX / VEC, NW = NG * GW;
+    constexpr int MAXST = (8 * NQ + NG - 1) / NG;  // stages of one cell that can fall to one group
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int nhp = nhp_of(p.nh), tabn = tabn_of(p.nh);
     const int NR = p.nh[1] * p.nh[2];       // rows of an octant chunk
@@ -204,41 +222,108 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
     const uint32_t tab_bytes = (uint32_t)tabn * (uint32_t)sizeof(T);
     const uint32_t cell_bytes = (uint32_t)rows_cell_bytes(sizeof(T), tabn);
     const int NS = p.ring_stages;
-    const RowsSmem s = rows_carve(smem_raw, sizeof(T), NS, slot_bytes, NW, tabn, NR);
+    const RowsSmem s = rows_map(sizeof(T), NS, slot_bytes, NW, tabn, NR);
+    const uint32_t sb = smem_u32(smem_raw);  // shared-space address of the map's origin
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     if (tid == 0) {
-        for (int i = 0; i < NS; i++) { mbar_init(&s.full[i], 1); mbar_init(&s.empty[i], NW); }
-        for (int i = 0; i < CELL_SLOTS; i++) { mbar_init(&s.cfull[i], 1); mbar_init(&s.cempty[i], NW); s.cnt[i] = 0; }
+        for (int i = 0; i < NS; i++) {
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + s.full) + i, 1);
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + s.empty) + i, GW);
+        }
+        for (int i = 0; i < CELL_SLOTS; i++) {
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + s.cfull) + i, 1);
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + s.cempty) + i, NW);
+            reinterpret_cast<int*>(smem_raw + s.cnt)[i] = 0;
+        }
+        reinterpret_cast<int*>(smem_raw + s.issued)[0] = reinterpret_cast<int*>(smem_raw + s.issued)[1] = 0;
         mbar_init_fence();
         if (blockIdx.x == 0) *p.counter_reset = 0;  // the other launch parity's cell counter
     }
     for (int r = tid; r < NR; r += blockDim.x)
-        s.ayz[r] = make_double2(p.vel->xi[1][p.nh[1] + r % p.nh[1]], p.vel->xi[2][p.nh[2] + r / p.nh[1]]);
+        reinterpret_cast<double2*>(smem_raw + s.ayz)[r] =
+            make_double2(p.vel->xi[1][p.nh[1] + r % p.nh[1]], p.vel->xi[2][p.nh[2] + r / p.nh[1]]);
     __syncthreads();
     const T* fin = reinterpret_cast<const T*>(p.f_in);
 
     if (warp == NW) {
-        // ------------------------------------------------ producer warp: cell tickets, headers, TMA copies
+        // ------------------------------------------------ producer warp: cell tickets, headers, factor tables, TMA copies
+        const int o_l = lane >> 2, t_l = lane & 3;
+        int slot = 0, gidx = 0;  // ring cursor and global index of the next slot (both producers count every slot)
+        uint32_t ph = 0;
+        auto skip = [&](int k) {
+            gidx += k;
+            slot += k;
+            while (slot >= NS) { slot -= NS; ph ^= 1u; }
+        };
+        // arm the slot for `bytes` and publish it; the caller's lanes then issue the copies
+        auto arm = [&](uint32_t bytes) {
+            smbar_wait(sb + s.empty + 8u * slot, ph ^ 1u);
+            if (lane == 0) {
+                smbar_arrive_expect_tx(sb + s.full + 8u * slot, bytes);
+                __threadfence_block();
+                ssts_i32_volatile(sb + s.issued, gidx + 1);
+            }
+            __syncwarp();
+        };
+        // issue octants [o0, o1) of cell `cur`; rec = this lane's word of the cell record, masks = 3 bits per octant
+        auto issue = [&](int cur, int rec, int masks, int o0, int o1) {
+            // lane (o,t): stream t of octant o -- t = 0 own chunk, t = 1..3 the upwind chunk on axis t-1
+            const int a = t_l > 0 ? t_l - 1 : 0;
+            const int dir = 2 * a + (1 - ((o_l >> a) & 1));
+            const int code = __shfl_sync(0xffffffffu, rec, dir * 4);
+            const int kind = code >> SRC_SHIFT;
+            const int64_t idx = code & SRC_INDEX_MASK;
+            const T* ptr = (t_l == 0) ? fin + (int64_t)cur * p.Nv + (int64_t)o_l * CH
+                                      : (kind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + idx * p.Nv
+                                            + (int64_t)(kind == SRC_MIRROR ? (o_l ^ (1 << a)) : o_l) * CH;
+            for (int o = o0; o < o1; o++) {
+                const int mask = (masks >> (3 * o)) & 7;
+                const int xdir = lane < 3 ? 2 * lane + (1 - ((o >> lane) & 1)) : 0;
+#pragma unroll
+                for (int q = 0; q < NQ; q++) {
+                    arm(slot_bytes);
+                    if (o_l == o)
+                        sbulk_g2s(sb + s.ring + slot * slot_bytes + t_l * piece_bytes, ptr + (size_t)q * pe, piece_bytes,
+                                  sb + s.full + 8u * slot);
+                    skip(1);
+                    if (mask) {
+                        // sources 1..3 of the axes in `mask` follow in three more slots (piece t = axis t)
+#pragma unroll 1
+                        for (int j = 1; j < 4; j++) {
+                            const int xcode = __shfl_sync(0xffffffffu, rec, xdir * 4 + j);
+                            arm((uint32_t)__popc(mask) * piece_bytes);
+                            if (lane < 3 && ((mask >> lane) & 1)) {
+                                const int xkind = xcode >> SRC_SHIFT;
+                                const int64_t xidx = xcode & SRC_INDEX_MASK;
+                                const T* xptr = (xkind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + xidx * p.Nv
+                                                + (int64_t)(xkind == SRC_MIRROR ? (o ^ (1 << lane)) : o) * CH;
+                                sbulk_g2s(sb + s.ring + slot * slot_bytes + lane * piece_bytes, xptr + (size_t)q * pe, piece_bytes,
+                                          sb + s.full + 8u * slot);
+                            }
+                            skip(1);
+                        }
+                    }
+                }
+            }
+        };
         auto fetch_async = [&]() -> int { return lane == 0 ? atomicAdd(p.counter, 1) : 0; };
         auto load_rec = [&](int cell) -> int {
             return cell < p.n_kin ? __ldg(reinterpret_cast<const int*>(p.cells + cell) + lane) : 0;
         };
-        int slot = 0;
-        uint32_t ph = 0;
-        auto advance = [&]() { if (++slot == NS) { slot = 0; ph ^= 1u; } };
         int cur = __shfl_sync(0xffffffffu, fetch_async(), 0);
         int rec = load_rec(cur);
-        int nxt_raw = 0;
-        const int o_l = lane >> 2, t_l = lane & 3;
         for (int ncell = 0;; ncell++) {
             const int cs = ncell % CELL_SLOTS;
-            int* hdr = reinterpret_cast<int*>(s.cells + (size_t)cs * cell_bytes);
-            mbar_wait(&s.cempty[cs], (uint32_t)(((ncell / CELL_SLOTS) & 1) ^ 1), 1);
+            int* hdr = reinterpret_cast<int*>(smem_raw + s.cells + (size_t)cs * cell_bytes);
+            smbar_wait(sb + s.cempty + 8u * cs, (uint32_t)(((ncell / CELL_SLOTS) & 1) ^ 1));
             if (cur >= p.n_kin) {
-                if (lane == 0) { hdr[2] = CK_STOP; mbar_arrive(&s.cfull[cs]); }
+                if (lane == 0) { hdr[2] = CK_STOP; smbar_arrive(sb + s.cfull + 8u * cs); }
                 break;
             }
+            // The next ticket is drawn now -- late enough that the cells in flight stay close in slab order, early
+            // enough that the atomic and the record load (two dependent global round trips) hide behind the copies.
+            const int nxt_raw = fetch_async();
             const int level = __shfl_sync(0xffffffffu, rec, 24), flags = __shfl_sync(0xffffffffu, rec, 25);
             const bool ringable = (flags & CELL_NOFLUID) != 0;
             // bit d: direction d has four (finer) sources instead of one
@@ -249,68 +334,29 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
             int mymask = 0;
 #pragma unroll
             for (int b = 0; b < 3; b++) mymask |= ((four >> (2 * b + (1 - ((lane >> b) & 1)))) & 1) << b;
-            if (lane < 8) hdr[4 + lane] = ringable ? mymask : 0;
-            if (lane == 0) { hdr[0] = cur; hdr[1] = level; hdr[2] = ringable ? CK_RING : CK_GATHER; }
+            if (!ringable || lane >= 8) mymask = 0;
+            int masks = mymask << (3 * (lane & 7)), mbits = (mymask ? 1 : 0) << (lane & 7);
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) { masks |= __shfl_xor_sync(0xffffffffu, masks, d); mbits |= __shfl_xor_sync(0xffffffffu, mbits, d); }
+            masks = __shfl_sync(0xffffffffu, masks, 0); mbits = __shfl_sync(0xffffffffu, mbits, 0);
+            hdr[HDR_REC + lane] = rec;
+            if (lane == 0) { hdr[0] = cur; hdr[1] = level; hdr[2] = ringable ? CK_RING : CK_GATHER; hdr[3] = mbits; hdr[4] = masks; }
             __syncwarp();
             if (lane == 0) {
+                const uint32_t cf = sb + s.cfull + 8u * cs;
                 if (p.collide) {
-                    mbar_arrive_expect_tx(&s.cfull[cs], tab_bytes);
-                    bulk_g2s(hdr + HDR_INTS, reinterpret_cast<const T*>(p.tabs) + (int64_t)cur * tabn, tab_bytes, &s.cfull[cs]);
+                    smbar_arrive_expect_tx(cf, tab_bytes);
+                    sbulk_g2s(sb + s.cells + cs * cell_bytes + HDR_INTS * 4, reinterpret_cast<const T*>(p.tabs) + (int64_t)cur * tabn,
+                              tab_bytes, cf);
                 } else {
-                    mbar_arrive(&s.cfull[cs]);
+                    smbar_arrive(cf);
                 }
             }
-            if (ringable) {
-                // lane (o,t): stream t of octant o -- t = 0 own chunk, t = 1..3 the upwind chunk on axis t-1
-                const int a = t_l > 0 ? t_l - 1 : 0;
-                const int dir = 2 * a + (1 - ((o_l >> a) & 1));
-                const int code = __shfl_sync(0xffffffffu, rec, dir * 4);
-                const int kind = code >> SRC_SHIFT;
-                const int64_t idx = code & SRC_INDEX_MASK;
-                const T* ptr = (t_l == 0) ? fin + (int64_t)cur * p.Nv + (int64_t)o_l * CH
-                                          : (kind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + idx * p.Nv
-                                                + (int64_t)(kind == SRC_MIRROR ? (o_l ^ (1 << a)) : o_l) * CH;
-                for (int o = 0; o < 8; o++) {
-                    // the next ticket is drawn late, so that the cells in flight stay consecutive in slab order
-                    if (o == 7) nxt_raw = fetch_async();
-                    const int mask = __shfl_sync(0xffffffffu, mymask, o);
-                    const int xdir = lane < 3 ? 2 * lane + (1 - ((o >> lane) & 1)) : 0;
-#pragma unroll
-                    for (int q = 0; q < NQ; q++) {
-                        mbar_wait(&s.empty[slot], ph ^ 1u, 2);
-                        if (lane == 0) mbar_arrive_expect_tx(&s.full[slot], slot_bytes);
-                        __syncwarp();
-                        if (o_l == o) {
-                            void* dst = s.ring + (size_t)slot * slot_bytes + (size_t)t_l * piece_bytes;
-                            bulk_g2s(dst, ptr + (size_t)q * pe, piece_bytes, &s.full[slot]);
-                        }
-                        advance();
-                        if (mask) {
-                            // sources 1..3 of the axes in `mask` follow in three more slots (piece t = axis t)
-#pragma unroll 1
-                            for (int j = 1; j < 4; j++) {
-                                const int xcode = __shfl_sync(0xffffffffu, rec, xdir * 4 + j);
-                                mbar_wait(&s.empty[slot], ph ^ 1u, 3);
-                                if (lane == 0) mbar_arrive_expect_tx(&s.full[slot], (uint32_t)__popc(mask) * piece_bytes);
-                                __syncwarp();
-                                if (lane < 3 && ((mask >> lane) & 1)) {
-                                    const int xkind = xcode >> SRC_SHIFT;
-                                    const int64_t xidx = xcode & SRC_INDEX_MASK;
-                                    const T* xptr = (xkind == SRC_TABLE ? reinterpret_cast<const T*>(p.tables) : fin) + xidx * p.Nv
-                                                    + (int64_t)(xkind == SRC_MIRROR ? (o ^ (1 << lane)) : o) * CH;
-                                    void* dst = s.ring + (size_t)slot * slot_bytes + (size_t)lane * piece_bytes;
-                                    bulk_g2s(dst, xptr + (size_t)q * pe, piece_bytes, &s.full[slot]);
-                                }
-                                advance();
-                            }
-                        }
-                    }
-                }
-            } else {
-                nxt_raw = fetch_async();
-            }
-            cur = __shfl_sync(0xffffffffu, nxt_raw, 0);
-            rec = load_rec(cur);
+            const int nxt = __shfl_sync(0xffffffffu, nxt_raw, 0);
+            const int nrec = load_rec(nxt);  // in flight while this cell's copies are issued
+            if (ringable) issue(cur, rec, masks, 0, 8);
+            cur = nxt;
+            rec = nrec;
         }
         return;
     }
@@ -319,145 +365,159 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
     const int g = warp / GW;
     const int r = (warp % GW) * 32 + lane;  // row inside a stage
     const bool active = r < NRQ;
-    int slot = 0, turn = 0;                 // turn = n mod NG
-    uint32_t ph = 0;
+    double ay[NQ], az[NQ];
+    int ry[NQ], rz[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; q++) {
+        const int row = active ? q * NRQ + r : 0;
+        const double2 yz = reinterpret_cast<const double2*>(smem_raw + s.ayz)[row];
+        ay[q] = yz.x; az[q] = yz.y;
+        ry[q] = row % p.nh[1]; rz[q] = row / p.nh[1];
+    }
+    const uint32_t inv_ns = (65536u + (uint32_t)NS - 1u) / (uint32_t)NS;  // x / NS = (x * inv_ns) >> 16 for x < 128
+    int slot0 = 0, gslot0 = 0, turn0 = 0;  // ring cursor, slots consumed so far, stage counter mod NG at the cell's start
+    uint32_t ph0 = 0;
     for (int ncell = 0;; ncell++) {
         const int cs = ncell % CELL_SLOTS;
-        const int* hdr = reinterpret_cast<const int*>(s.cells + (size_t)cs * cell_bytes);
-        mbar_wait(&s.cfull[cs], (uint32_t)((ncell / CELL_SLOTS) & 1), 4);
-        const int kind = hdr[2];
+        const uint32_t hdr = s.cells + cs * cell_bytes;
+        smbar_wait(sb + s.cfull + 8u * cs, (uint32_t)((ncell / CELL_SLOTS) & 1));
+        const int4 h0 = *reinterpret_cast<const int4*>(smem_raw + hdr);
+        const int kind = h0.z;
         if (kind == CK_STOP) break;
-        const int cell = hdr[0];
-        const T* tab = reinterpret_cast<const T*>(hdr + HDR_INTS);
-        const double dth = p.dt * p.inv_len * (double)(1 << hdr[1]);  // dt / h
-        int masks = 0;
-#pragma unroll
-        for (int o = 0; o < 8; o++) masks |= hdr[4 + o] << (3 * o);
+        const int cell = h0.x;
+        const T* tab = reinterpret_cast<const T*>(smem_raw + hdr + HDR_INTS * 4);
+        const double dth = p.dt * p.inv_len * (double)(1 << h0.y);  // dt / h
+        const int mbits = h0.w;  // 1 bit per octant: it has a 2:1 upwind face
+        const int masks = *reinterpret_cast<const int*>(smem_raw + hdr + 16);  // 3 bits per octant: on which axes
         RowCtx<T, NQ> rc;
         rc.omega = p.collide ? tab[6 * nhp] : T(0);
         const double om1 = 1.0 - (double)rc.omega;
         rc.sx = (T)(om1 * dth);
 #pragma unroll
         for (int q = 0; q < NQ; q++) {
-            const int row = active ? q * NRQ + r : 0;
-            const double2 yz = s.ayz[row];
-            rc.ay[q] = yz.x; rc.az[q] = yz.y;
-            rc.ry[q] = row % p.nh[1]; rc.rz[q] = row / p.nh[1];
-            rc.base[q] = (T)(om1 * (1.0 - dth * (yz.x + yz.y)));
-            rc.cy[q] = (T)(om1 * dth * yz.x);
-            rc.cz[q] = (T)(om1 * dth * yz.y);
+            rc.base[q] = (T)(om1 * (1.0 - dth * (ay[q] + az[q])));
+            rc.cy[q] = (T)(om1 * dth * ay[q]);
+            rc.cz[q] = (T)(om1 * dth * az[q]);
         }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)cell * p.Nv;
-        const int* rec = reinterpret_cast<const int*>(p.cells + cell);
-        double acc[35];
+        // this group's stages of the cell: first, first + NG, ...  (stage = octant * NQ + row block)
+        int first = g - turn0;
+        if (first < 0) first += NG;
+        double S[MAXST][4];  // the row sums of this thread's stages (registers: the loops over them are unrolled)
+        int so[MAXST];
 #pragma unroll
-        for (int i = 0; i < 35; i++) acc[i] = 0.0;
-#pragma unroll 1
-        for (int o = 0; o < 8; o++) {
-            const int mask = (masks >> (3 * o)) & 7;
-#pragma unroll
-            for (int q = 0; q < NQ; q++) {
-                const bool mine = turn == g;
-                if (++turn == NG) turn = 0;
+        for (int i = 0; i < MAXST; i++) {
+            const int stg = first + i * NG;
+            so[i] = -1;
+            S[i][0] = S[i][1] = S[i][2] = S[i][3] = 0.0;
+            if (stg < 8 * NQ) {
+                const int o = stg / NQ, q = stg % NQ;
+                so[i] = stg;
+                const int mask = (masks >> (3 * o)) & 7;
+                const T* gxrow = tab + (o & 1) * nhp;
+                T* const gdst = gcell + (int64_t)o * CH + (int64_t)(q * NRQ + r) * NHX;
+                T wb = T(0);
+                if (p.collide) wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rz[q]] * tab[(2 + ((o >> 1) & 1)) * nhp + ry[q]]);
                 if (kind == CK_RING) {
-                    if (mine) {
-                        mbar_wait(&s.full[slot], ph, 5);
-                        T* const st = reinterpret_cast<T*>(s.ring + (size_t)slot * slot_bytes) + (size_t)r * NHX;
-                        if (mask) {
-                            // 2:1 face (reading G3): the next three slots bring sources 1..3 of the axes in `mask`; they
-                            // are added, in order, onto source 0 where it lies in this slot (a thread touches its own
-                            // row only)
-                            int sl = slot;
-                            uint32_t sp = ph;
+                    // ring slots taken by the stages before this one: one each, four where the octant has a 2:1 face
+                    const int before = stg + 3 * (NQ * __popc(mbits & ((1 << o) - 1)) + (mask ? q : 0));
+                    const int lin = slot0 + before;
+                    const int wraps = (int)(((uint32_t)lin * inv_ns) >> 16);
+                    int slot = lin - wraps * NS;
+                    uint32_t ph = ph0 ^ (uint32_t)(wraps & 1);
+                    // the producer must have armed the stage's last slot before its barrier's parity means anything
+                    const int need = gslot0 + before + (mask ? 4 : 1);
+                    while (slds_i32_volatile(sb + s.issued) < need) __nanosleep(64);
+                    __threadfence_block();
+                    smbar_wait(sb + s.full + 8u * slot, ph);
+                    T* const st = reinterpret_cast<T*>(smem_raw + s.ring + (size_t)slot * slot_bytes) + (size_t)r * NHX;
+                    if (mask) {
+                        // 2:1 face (reading G3): the next three slots bring sources 1..3 of the axes in `mask`; they are
+                        // added, in order, onto source 0 where it lies in this slot (a thread touches its own row only)
+                        int sl = slot;
+                        uint32_t sp = ph;
 #pragma unroll 1
-                            for (int j = 1; j < 4; j++) {
-                                if (++sl == NS) { sl = 0; sp ^= 1u; }
-                                mbar_wait(&s.full[sl], sp, 6);
-                                if (active) {
-                                    const T* se = reinterpret_cast<const T*>(s.ring + (size_t)sl * slot_bytes) + (size_t)r * NHX;
-#pragma unroll 1
-                                    for (int t = 0; t < 3; t++) {
-                                        if ((mask >> t) & 1) {
-#pragma unroll
-                                            for (int jj = 0; jj < RV; jj++) {
-                                                T v[VEC], x[VEC];
-                                                lds16(se + t * pe + jj * VEC, v);
-                                                lds16(st + (t + 1) * pe + jj * VEC, x);
-#pragma unroll
-                                                for (int i = 0; i < VEC; i++) x[i] += v[i];
-                                                sts16(st + (t + 1) * pe + jj * VEC, x);
-                                            }
-                                        }
-                                    }
-                                }
-                                __syncwarp();
-                                if (lane == 0) mbar_arrive(&s.empty[sl]);
-                            }
-                            if (active) {  // each of the four sources weighs 1/4
+                        for (int j = 1; j < 4; j++) {
+                            if (++sl == NS) { sl = 0; sp ^= 1u; }
+                            smbar_wait(sb + s.full + 8u * sl, sp);
+                            if (active) {
+                                const T* se = reinterpret_cast<const T*>(smem_raw + s.ring + (size_t)sl * slot_bytes) + (size_t)r * NHX;
 #pragma unroll 1
                                 for (int t = 0; t < 3; t++) {
                                     if ((mask >> t) & 1) {
 #pragma unroll
                                         for (int jj = 0; jj < RV; jj++) {
-                                            T x[VEC];
+                                            T v[VEC], x[VEC];
+                                            lds16(se + t * pe + jj * VEC, v);
                                             lds16(st + (t + 1) * pe + jj * VEC, x);
 #pragma unroll
-                                            for (int i = 0; i < VEC; i++) x[i] *= T(0.25);
+                                            for (int ii = 0; ii < VEC; ii++) x[ii] += v[ii];
                                             sts16(st + (t + 1) * pe + jj * VEC, x);
                                         }
                                     }
                                 }
                             }
-                        }
-                        if (active) {
-                            const T wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rc.rz[q]] * tab[(2 + ((o >> 1) & 1)) * nhp + rc.ry[q]]);
-                            double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
-                            row_from_ring<T, NHX, NQ>(p, rc, q, wb, st, pe, tab + (o & 1) * nhp,
-                                                      gcell + (int64_t)o * CH + (int64_t)(q * NRQ + r) * NHX, s0, s1, s2, s3);
-                            fold_row_rt(o, s0, s1, s2, s3, rc.ay[q], rc.az[q], acc);
-                        }
-                        // a slot written with ordinary stores: order them before the bulk copy that refills it
-                        if (mask) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&s.empty[slot]);
-                    } else {
-                        // Not this group's stage: observe and release its slots all the same.  Every warp then sees
-                        // every phase of every slot, so a group can never run a lap ahead of a barrier it skipped
-                        // (its parity test would pass on a slot that has not been filled yet).
-                        int sl = slot;
-                        uint32_t sp = ph;
-                        for (int j = 0; j < (mask ? 4 : 1); j++) {
-                            mbar_wait(&s.full[sl], sp, 7);
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(&s.empty[sl]);
-                            if (++sl == NS) { sl = 0; sp ^= 1u; }
+                            if (lane == 0) smbar_arrive(sb + s.empty + 8u * sl);
+                        }
+                        if (active) {  // each of the four sources weighs 1/4
+#pragma unroll 1
+                            for (int t = 0; t < 3; t++) {
+                                if ((mask >> t) & 1) {
+#pragma unroll
+                                    for (int jj = 0; jj < RV; jj++) {
+                                        T x[VEC];
+                                        lds16(st + (t + 1) * pe + jj * VEC, x);
+#pragma unroll
+                                        for (int ii = 0; ii < VEC; ii++) x[ii] *= T(0.25);
+                                        sts16(st + (t + 1) * pe + jj * VEC, x);
+                                    }
+                                }
+                            }
                         }
                     }
-                    const int adv = mask ? 4 : 1;
-                    slot += adv;
-                    if (slot >= NS) { slot -= NS; ph ^= 1u; }
-                } else if (mine && active) {
-                    const T wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rc.rz[q]] * tab[(2 + ((o >> 1) & 1)) * nhp + rc.ry[q]]);
-                    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
-                    row_from_gather<T, NHX, NQ>(p, rc, q, wb, o, CH, q * NRQ + r, rec, fin, cell, tab + (o & 1) * nhp,
-                                                gcell + (int64_t)o * CH + (int64_t)(q * NRQ + r) * NHX, s0, s1, s2, s3);
-                    fold_row_rt(o, s0, s1, s2, s3, rc.ay[q], rc.az[q], acc);
+                    // a slot written with ordinary stores: order them before the bulk copy that refills it
+                    if (mask) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    row_from_ring<T, NHX, NQ, EARLY>(p, rc, q, wb, st, pe, gxrow, gdst, active, lane, sb + s.empty + 8u * slot,
+                                                     S[i][0], S[i][1], S[i][2], S[i][3]);
+                } else if (active) {
+                    row_from_gather<T, NHX, NQ>(p, rc, q, wb, o, CH, q * NRQ + r, ry[q], rz[q], reinterpret_cast<const int*>(p.cells + cell),
+                                                fin, cell, gxrow, gdst, S[i][0], S[i][1], S[i][2], S[i][3]);
                 }
             }
         }
-        // the warp's partial sums; the warp that delivers last adds all of them up and writes the cell's sums
-        double* red = s.red + ((size_t)cs * NW + warp) * SUMS_STRIDE;
-        warp_store_sums(acc, red, lane);
+        if (kind == CK_RING) {
+            const int total = 8 * NQ + 3 * NQ * __popc(mbits);
+            const int lin = slot0 + total;
+            const int wraps = (int)(((uint32_t)lin * inv_ns) >> 16);
+            slot0 = lin - wraps * NS;
+            ph0 ^= (uint32_t)(wraps & 1);
+            gslot0 += total;
+        }
+        turn0 = (turn0 + 8 * NQ) % NG;
+        // fold the y/z weights and signs into the row sums (a2'), then the warp's partial sums; the warp that delivers
+        // last adds all of them up and writes the cell's sums
+        double acc[35];
+#pragma unroll
+        for (int i = 0; i < 35; i++) acc[i] = 0.0;
+#pragma unroll
+        for (int i = 0; i < MAXST; i++) {
+            if (so[i] >= 0 && active) {
+                const int q = so[i] % NQ;
+                fold_row_rt(so[i] / NQ, S[i][0], S[i][1], S[i][2], S[i][3], NQ > 1 && q ? ay[NQ - 1] : ay[0], NQ > 1 && q ? az[NQ - 1] : az[0], acc);
+            }
+        }
+        warp_store_sums(acc, reinterpret_cast<double*>(smem_raw + s.red) + ((size_t)cs * NW + warp) * SUMS_STRIDE, lane);
         __threadfence_block();
         __syncwarp();
         int last = 0;
-        if (lane == 0) last = atomicAdd(&s.cnt[cs], 1) == NW - 1;
+        if (lane == 0) last = atomicAdd(reinterpret_cast<int*>(smem_raw + s.cnt) + cs, 1) == NW - 1;
         last = __shfl_sync(0xffffffffu, last, 0);
         if (last) {
             __threadfence_block();
             if (lane < SUMS_STRIDE / 2) {
                 double2 t = make_double2(0.0, 0.0);
-                const double2* src = reinterpret_cast<const double2*>(s.red + (size_t)cs * NW * SUMS_STRIDE) + lane;
+                const double2* src = reinterpret_cast<const double2*>(smem_raw + s.red + (size_t)cs * NW * SUMS_STRIDE * 8) + lane;
 #pragma unroll
                 for (int w = 0; w < NW; w++) {
                     const double2 v = src[w * (SUMS_STRIDE / 2)];
@@ -465,33 +525,45 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                 }
                 reinterpret_cast<double2*>(p.sums_out + (int64_t)cell * SUMS_STRIDE)[lane] = t;
             }
-            if (lane == 0) s.cnt[cs] = 0;
+            if (lane == 0) reinterpret_cast<int*>(smem_raw + s.cnt)[cs] = 0;
             __syncwarp();
         }
-        if (lane == 0) mbar_arrive(&s.cempty[cs]);
+        if (lane == 0) smbar_arrive(sb + s.cempty + 8u * cs);
     }
 }
 
 constexpr size_t ROWS_SMEM_MAX = 227 * 1024;
 
-// the instantiations: (storage type, nh_x, warps per group, groups, row blocks per octant chunk)
-struct RowsVariant { int storage, nhx, gw, ng, nq; };
+// the instantiations: (storage type, nh_x, warps per group, groups, row blocks per octant chunk, early release);
+// the first one that fits is used unless UFS_DVM_ROWS picks another by index (timing experiments)
+struct RowsVariant { int storage, nhx, gw, ng, nq, early; };
 constexpr RowsVariant ROWS_VARIANTS[] = {
-    {UFS_STORE_F32, 12, 5, 3, 1},
-    {UFS_STORE_F64, 12, 3, 5, 2},
-    {UFS_STORE_F64, 6, 2, 4, 1},
+    {UFS_STORE_F32, 12, 5, 3, 1, 0},
+    {UFS_STORE_F64, 12, 3, 5, 2, 0},
+    {UFS_STORE_F64, 6, 2, 4, 1, 1},
+    {UFS_STORE_F32, 12, 5, 2, 1, 1},
+    {UFS_STORE_F32, 12, 3, 5, 2, 0},
+    {UFS_STORE_F32, 12, 3, 4, 2, 1},
 };
-const RowsVariant* rows_variant(int storage, const VelLayout& v) {
-    if (!v.fast) return nullptr;
+constexpr int N_ROWS_VARIANTS = sizeof(ROWS_VARIANTS) / sizeof(ROWS_VARIANTS[0]);
+bool rows_variant_fits(const RowsVariant& rv, int storage, const VelLayout& v) {
     const int nr = v.nh[1] * v.nh[2];
-    for (const RowsVariant& rv : ROWS_VARIANTS)
-        if (rv.storage == storage && rv.nhx == v.nh[0] && nr % rv.nq == 0 && nr / rv.nq <= rv.gw * 32) return &rv;
-    return nullptr;
+    return rv.storage == storage && rv.nhx == v.nh[0] && nr % rv.nq == 0 && nr / rv.nq <= rv.gw * 32;
+}
+int rows_variant(int storage, const VelLayout& v) {
+    if (!v.fast) return -1;
+    if (const char* e = std::getenv("UFS_DVM_ROWS")) {
+        const int i = std::atoi(e);
+        if (i >= 0 && i < N_ROWS_VARIANTS && rows_variant_fits(ROWS_VARIANTS[i], storage, v)) return i;
+    }
+    for (int i = 0; i < N_ROWS_VARIANTS; i++)
+        if (rows_variant_fits(ROWS_VARIANTS[i], storage, v)) return i;
+    return -1;
 }
 
-template <typename T, int NHX, int GW, int NG, int NQ>
+template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY>
 cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
-    auto k = k_rows<T, NHX, GW, NG, NQ>;
+    auto k = k_rows<T, NHX, GW, NG, NQ, EARLY>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_kin < plan.grid ? p.n_kin : plan.grid;
@@ -504,8 +576,9 @@ cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStrea
 // Launch geometry of the row kernel for this storage type / velocity grid, or false if no instantiation fits (the
 // one-vector-per-thread kernel of step_stream.cu, then the one-CTA-per-cell kernels of kernels.cu, take over).
 bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan) {
-    const RowsVariant* rv = rows_variant(storage, v);
-    if (!rv) return false;
+    const int vi = rows_variant(storage, v);
+    if (vi < 0) return false;
+    const RowsVariant* rv = &ROWS_VARIANTS[vi];
     for (int a = 0; a < 3; a++)
         if (v.nv[a] > 32) return false;
     StepLaunch base{};
@@ -519,12 +592,15 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan) 
     int ns = 16;
     while (ns >= 4 && rows_smem_bytes(elem, ns, slot, nw, tabn, nr) > ROWS_SMEM_MAX) ns--;
     if (ns < 4) return false;  // a 2:1 face needs four slots in flight at once
+    if (const char* e = std::getenv("UFS_DVM_NS")) { const int f = std::atoi(e); if (f >= 4 && f < ns) ns = f; }
     *plan = base;
     plan->ring = 3;
+    plan->ncw = vi;            // which instantiation
     plan->stages = ns;
     plan->threads = (nw + 1) * 32;
     plan->smem_bytes = (int32_t)rows_smem_bytes(elem, ns, slot, nw, tabn, nr);
     plan->grid = sm_count;
+    if (const char* e = std::getenv("UFS_DVM_GRID")) { const int f = std::atoi(e); if (f >= 1 && f < sm_count) plan->grid = f; }
     return true;
 }
 
@@ -532,14 +608,19 @@ cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p
     if (p.n_kin == 0) return cudaSuccess;
     cudaError_t e = launch_prep(storage, p, st);
     if (e != cudaSuccess) return e;
-    if (storage == UFS_STORE_F32) return launch_rows_t<float, 12, 5, 3, 1>(plan, p, st);
-    if (p.nh[0] == 12) return launch_rows_t<double, 12, 3, 5, 2>(plan, p, st);
-    return launch_rows_t<double, 6, 2, 4, 1>(plan, p, st);
+    switch (plan.ncw) {
+        case 0: return launch_rows_t<float, 12, 5, 3, 1, false>(plan, p, st);
+        case 1: return launch_rows_t<double, 12, 3, 5, 2, false>(plan, p, st);
+        case 2: return launch_rows_t<double, 6, 2, 4, 1, true>(plan, p, st);
+        case 3: return launch_rows_t<float, 12, 5, 2, 1, true>(plan, p, st);
+        case 4: return launch_rows_t<float, 12, 3, 5, 2, false>(plan, p, st);
+        case 5: return launch_rows_t<float, 12, 3, 4, 2, true>(plan, p, st);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 }  // namespace ufs
+
 #ifdef UFS_DEBUG_WAIT
-extern "C" int ufs_dvm_debug_read(int* out) {
-    return (int)cudaMemcpyFromSymbol(out, ufs::g_dbg, sizeof(int) * 8);
-}
+extern "C" int ufs_dvm_debug_read(int* out) { return (int)cudaMemcpyFromSymbol(out, ufs::g_dbg, sizeof(int) * 8); }
 #endif
