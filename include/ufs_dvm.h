@@ -135,6 +135,13 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void *f_host_in, void *f_host_out, doubl
 /* Number of kernels this handle has launched so far (step + moments kernels). */
 int64_t ufs_dvm_launch_count(ufs_dvm_t h);
 
+/* Measurement aid.  ufs_dvm_profile(h, 1) makes the following steps (at most 64) bracket their main kernel -- the
+ * streaming pass that reads and writes f -- with CUDA events on the handle's stream; ufs_dvm_profile(h, 0) stops.
+ * ufs_dvm_kernel_ms synchronises the stream and returns (HOST outputs) the mean duration in ms of those launches
+ * and their number.  The small per-cell Newton kernel that precedes the pass is not inside the bracket. */
+int ufs_dvm_profile(ufs_dvm_t h, int enable);
+int ufs_dvm_kernel_ms(ufs_dvm_t h, double *mean_ms, int32_t *n_launches);
+
 /* Launch geometry of the step kernel: threads per CTA, dynamic shared memory per CTA, vector width in
  * elements, and 1 if the octant fast path is used (0 = generic per-slot path).  HOST outputs. */
 int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t *threads, int32_t *smem_bytes, int32_t *vec, int32_t *fast);

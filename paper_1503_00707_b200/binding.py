@@ -20,7 +20,7 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
-           "ufs_dvm_last_error", "ufs_dvm_f_changed"]
+           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -54,6 +54,8 @@ def lib() -> C.CDLL:
         L.ufs_dvm_destroy.argtypes = [vp]
         L.ufs_dvm_current.argtypes = [vp]
         L.ufs_dvm_f_changed.argtypes = [vp]
+        L.ufs_dvm_profile.argtypes = [vp, C.c_int]
+        L.ufs_dvm_kernel_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
         L.ufs_dvm_layout.argtypes = [vp, C.POINTER(C.c_int64), i64p, vp]
         L.ufs_dvm_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp]
         L.ufs_dvm_boundary_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
@@ -138,6 +140,16 @@ def ufs_dvm_current(h) -> int:
 
 def ufs_dvm_f_changed(h):
     _check(h, lib().ufs_dvm_f_changed(h))
+
+
+def ufs_dvm_profile(h, enable: bool):
+    _check(h, lib().ufs_dvm_profile(h, int(bool(enable))))
+
+
+def ufs_dvm_kernel_ms(h):
+    ms, n = C.c_double(0.0), C.c_int32(0)
+    _check(h, lib().ufs_dvm_kernel_ms(h, C.byref(ms), C.byref(n)))
+    return float(ms.value), int(n.value)
 
 
 def ufs_dvm_layout(h, Nv: int):

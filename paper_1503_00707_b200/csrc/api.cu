@@ -34,10 +34,13 @@ struct ufs_dvm_s {
     void* d_tabs = nullptr;
     bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
-    int l2_mode = 0;
-    int ticket_mode = 1;
     StepLaunch plan{};
     int64_t launches = 0;
+    // optional timing of the main kernel of each step (ufs_dvm_profile)
+    static constexpr int MAX_PROF = 64;
+    cudaEvent_t prof_ev[MAX_PROF][2] = {};
+    int prof_n = 0;
+    bool prof_on = false;
     int sticky = UFS_DVM_OK;
     std::string err;
 };
@@ -92,8 +95,6 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.counter = h->d_counter + h->parity;
     p.counter_reset = h->d_counter + (h->parity ^ 1);
     p.ring_stages = h->plan.stages;
-    p.l2_mode = h->l2_mode;
-    p.ticket_mode = h->ticket_mode;
     p.sums_in = h->d_sums[h->cur];
     p.sums_out = h->d_sums[h->cur ^ 1];
     p.ghost_sums = h->d_ghost_sums;
@@ -195,29 +196,18 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     CU(cudaMemsetAsync(h->d_counter, 0, 8, h->stream), "clear cell counters");
     // kernel choice: the persistent TMA ring kernel where the velocity grid fits it, else one CTA per cell
     // (UFS_DVM_KERNEL=cell forces the latter: A/B timing and tests)
-    if (const char* l2 = std::getenv("UFS_DVM_L2")) h->l2_mode = std::atoi(l2);
-    if (const char* tk = std::getenv("UFS_DVM_TICKET")) h->ticket_mode = std::atoi(tk);
-    // UFS_DVM_KERNEL = stream (default) | ring | cell : A/B timing and tests of the older kernels
+    // Kernel choice: the streaming step (one row per thread, else one vector per thread) where the velocity grid fits
+    // it, else one CTA per cell.  UFS_DVM_KERNEL = stream | cell forces the older variants (A/B timing, tests).
     const char* force = std::getenv("UFS_DVM_KERNEL");
     const bool want_cell = force && std::strcmp(force, "cell") == 0;
-    const bool want_ring = force && std::strcmp(force, "ring") == 0;
+    const bool want_vec = force && std::strcmp(force, "stream") == 0;
     if (!want_cell) {
         int dev = 0, sms = 0;
         CU(cudaGetDevice(&dev), "get device");
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
         StepLaunch cand{};
-        const bool want_vec = force && std::strcmp(force, "stream") == 0;   // the one-vector-per-thread variant
-        if (!want_ring && !want_vec && rows_plan(h->storage, v, sms, &cand)) {
-            h->plan = cand;
-        } else if (!want_ring && stream_plan(h->storage, v, sms, &cand)) {
-            h->plan = cand;
-        } else if (ring_plan(h->storage, v, sms, &cand)) {
-            const int occ = ring_occupancy(h->storage, cand);
-            if (occ > 0) {
-                cand.grid = sms * occ;
-                h->plan = cand;
-            }
-        }
+        if (!want_vec && rows_plan(h->storage, v, sms, &cand)) h->plan = cand;
+        else if (stream_plan(h->storage, v, sms, &cand)) h->plan = cand;
     }
     if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
@@ -262,7 +252,16 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
             h->sums_valid = true;
             h->launches++;
         }
-        CU(launch_step(h->storage, h->plan, p, h->stream), "step kernel launch");
+        StepLaunch plan = h->plan;
+        plan.ev0 = plan.ev1 = nullptr;
+        if (h->prof_on && h->prof_n < ufs_dvm_s::MAX_PROF) {
+            for (int e = 0; e < 2; e++)
+                if (!h->prof_ev[h->prof_n][e]) CU(cudaEventCreate(&h->prof_ev[h->prof_n][e]), "create event");
+            plan.ev0 = h->prof_ev[h->prof_n][0];
+            plan.ev1 = h->prof_ev[h->prof_n][1];
+            h->prof_n++;
+        }
+        CU(launch_step(h->storage, plan, p, h->stream), "step kernel launch");
         h->cur ^= 1;
         h->parity ^= 1;
         if (h->mesh.n_kin > 0) h->launches += (stream && p.collide) ? 2 : 1;
@@ -312,6 +311,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
+        for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
     }
     delete h;
     return rc;
@@ -380,6 +380,28 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, doubl
 
 int64_t ufs_dvm_launch_count(ufs_dvm_t h) { return h ? h->launches : 0; }
 
+int ufs_dvm_profile(ufs_dvm_t h, int enable) {
+    if (!h) return UFS_DVM_EINVAL;
+    h->prof_on = enable != 0;
+    h->prof_n = 0;
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_kernel_ms(ufs_dvm_t h, double* mean_ms, int32_t* n_launches) {
+    if (!h || !mean_ms || !n_launches) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    CU(cudaStreamSynchronize(h->stream), "stream synchronize");
+    double sum = 0.0;
+    for (int i = 0; i < h->prof_n; i++) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, h->prof_ev[i][0], h->prof_ev[i][1]), "event elapsed time");
+        sum += ms;
+    }
+    *n_launches = h->prof_n;
+    *mean_ms = h->prof_n ? sum / h->prof_n : 0.0;
+    return UFS_DVM_OK;
+}
+
 int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int32_t* vec, int32_t* fast) {
     if (!h) return UFS_DVM_EINVAL;
     if (threads) *threads = h->plan.threads;
@@ -391,7 +413,7 @@ int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int3
 
 const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
     if (!h) return "";
-    return h->plan.ring == 3 ? "k_rows" : h->plan.ring == 2 ? "k_stream" : h->plan.ring ? "k_step_ring" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
+    return h->plan.ring == 3 ? "k_rows" : h->plan.ring == 2 ? "k_stream" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
 }
 
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }

@@ -571,17 +571,21 @@ cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p
     if (p.n_kin == 0) return cudaSuccess;
     if (plan.ring == 3) return launch_rows(storage, plan, p, st);
     if (plan.ring == 2) return launch_stream(storage, plan, p, st);
-    if (plan.ring) return launch_ring(storage, plan, p, st);
+    if (plan.ev0) cudaEventRecord(plan.ev0, st);
+    cudaError_t e;
     if (plan.fast) {
         if (storage == UFS_STORE_F32) {
-            if (plan.vec == 4) return launch_fast<float, 4>(plan, p, st);
-            if (plan.vec == 2) return launch_fast<float, 2>(plan, p, st);
-            return launch_fast<float, 1>(plan, p, st);
+            if (plan.vec == 4) e = launch_fast<float, 4>(plan, p, st);
+            else if (plan.vec == 2) e = launch_fast<float, 2>(plan, p, st);
+            else e = launch_fast<float, 1>(plan, p, st);
+        } else {
+            e = plan.vec == 2 ? launch_fast<double, 2>(plan, p, st) : launch_fast<double, 1>(plan, p, st);
         }
-        if (plan.vec == 2) return launch_fast<double, 2>(plan, p, st);
-        return launch_fast<double, 1>(plan, p, st);
+    } else {
+        e = storage == UFS_STORE_F32 ? launch_generic<float>(plan, p, st) : launch_generic<double>(plan, p, st);
     }
-    return storage == UFS_STORE_F32 ? launch_generic<float>(plan, p, st) : launch_generic<double>(plan, p, st);
+    if (plan.ev1) cudaEventRecord(plan.ev1, st);
+    return e;
 }
 
 cudaError_t launch_moments(int storage, const StepParams& p, const void* f, double* mom, cudaStream_t st) {

@@ -31,11 +31,9 @@ struct StepParams {
     int32_t nv[3], nh[3];
     int32_t collide;            // 0: Kn = inf, pure transport
     double dt, w, inv_len, inv_kn, visc_exp, nu_pref;
-    int32_t* counter;           // ring kernel: cell counter of this launch (zero at launch)
-    int32_t* counter_reset;     // ring kernel: the other launch parity's counter, zeroed by this launch
-    int32_t ring_stages;        // ring kernel: stages in the shared-memory ring
-    int32_t l2_mode;            // ring kernel: L2 eviction hints on the bulk loads (0 none; see step_ring.cu)
-    int32_t ticket_mode;        // ring kernel: how cells are handed to CTAs (see step_ring.cu)
+    int32_t* counter;           // streaming kernels: cell-ticket counter of this launch (zero at launch)
+    int32_t* counter_reset;     // the other launch parity's counter, zeroed by this launch
+    int32_t ring_stages;        // slots in the shared-memory ring
     // streaming step (step_stream.cu)
     const double* sums_in;      // [n_kin][SUMS_STRIDE] velocity sums of f_in
     double* sums_out;           // [n_kin][SUMS_STRIDE] velocity sums of f_out
@@ -52,9 +50,9 @@ constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used
 struct StepLaunch {
     int32_t threads, smem_bytes, vec, fast;
     int32_t ring;                  // 3: streaming step, one row per thread (step_rows.cu), 2: streaming step, one
-                                   // vector per thread (step_stream.cu), 1: TMA ring kernel with an on-chip slab
-                                   // (step_ring.cu), 0: one CTA per cell (kernels.cu)
+                                   // vector per thread (step_stream.cu), 0: one CTA per cell (kernels.cu)
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
+    cudaEvent_t ev0, ev1;          // if set: recorded on the stream right before / after the main kernel of the step
 };
 
 // per-axis table stride (nodes rounded up to a multiple of 4)
@@ -67,12 +65,6 @@ __host__ __device__ inline int nvp_of(const int32_t nv[3]) {
 // Chooses the kernel variant for this storage type / grid and returns its launch geometry, or an
 // error (negative) if the slab does not fit on chip.
 int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** why);
-
-// step_ring.cu: geometry of the persistent TMA ring kernel for this storage type / grid (false: not
-// applicable), and its launcher.
-bool ring_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
-int ring_occupancy(int storage, const StepLaunch& plan);
-cudaError_t launch_ring(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 
 // step_stream.cu: the streaming step (k_prep + k_stream), the sums of a freshly written f, moments from sums.
 bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);

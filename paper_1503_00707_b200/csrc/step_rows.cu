@@ -567,7 +567,9 @@ cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStrea
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_kin < plan.grid ? p.n_kin : plan.grid;
+    if (plan.ev0) cudaEventRecord(plan.ev0, st);
     k<<<grid, (NG * GW + 1) * 32, plan.smem_bytes, st>>>(p);
+    if (plan.ev1) cudaEventRecord(plan.ev1, st);
     return cudaGetLastError();
 }
 

@@ -697,7 +697,9 @@ cudaError_t launch_stream_t(const StepLaunch& plan, const StepParams& p, cudaStr
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_kin < plan.grid ? p.n_kin : plan.grid;
+    if (plan.ev0) cudaEventRecord(plan.ev0, st);
     k<<<grid, (STREAM_NCW + 2) * 32, plan.smem_bytes, st>>>(p);
+    if (plan.ev1) cudaEventRecord(plan.ev1, st);
     return cudaGetLastError();
 }
 
