@@ -113,6 +113,21 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def aggregate_over_ranks(ms_local: float, units_local: float, device=None):
+    """Whole-job figures of N independent replicas: the slowest rank's device time and the
+    units all ranks processed.  Works on any initialised process group (nccl on the GPU box, gloo in the CPU test);
+    without one it returns its arguments."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return ms_local, units_local
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    u = torch.tensor([units_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 def workload_config(case, args):
     return {"workload": f"{args.workload}: {case.name}, {int((case.kind == 0).sum())} kinetic leaves "
                         f"(levels {int(case.level.min())}-{int(case.level.max())}), velocity grid "
@@ -182,9 +197,8 @@ def main():
             B.ufs_dvm_run_host(st.h, host_in.data_ptr(), None, st.mom.data_ptr(), mom_host.data_ptr(), dt, args.steps)
             torch.cuda.synchronize(dev)
             t_e2e = time.perf_counter() - t0
-            if world > 1:
-                tt = torch.tensor([t_e2e], device=dev); dist.all_reduce(tt, op=dist.ReduceOp.MAX); t_e2e = float(tt.item())
-            e2e = {"value": world * n_kin * Nv * args.steps / t_e2e, "unit": UNIT,
+            t_e2e, units_e2e = aggregate_over_ranks(t_e2e, float(n_kin * Nv * args.steps), dev)
+            e2e = {"value": units_e2e / t_e2e, "unit": UNIT,
                    "h2d_bytes_per_step": n_kin * Nv * elem / args.steps, "d2h_bytes_per_step": n_kin * 40 / args.steps,
                    "seconds": t_e2e,
                    "what": "ufs_dvm_run_host: pinned host f -> device, K steps, moments, moments -> host"}
@@ -211,10 +225,9 @@ def main():
     B.ufs_dvm_profile(st.h, False)
     launches = B.ufs_dvm_launch_count(st.h) - launches0
     st.sync()                                   # raises on a sticky CUDA / Newton error
-    if world > 1:
-        tt = torch.tensor([ms], device=dev); dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = float(tt.item())
-    updates = n_kin * Nv * args.steps
-    value = world * updates / (ms * 1e-3)
+    ms_local = ms
+    ms, updates_all = aggregate_over_ranks(ms, float(n_kin * Nv * args.steps), dev)
+    value = updates_all / (ms * 1e-3)
 
     # ---- roofline of the dominant kernel (the streaming pass over f): its own launches, timed by events ----
     peak, peak_src = peaks()
@@ -227,7 +240,7 @@ def main():
                 "traffic": None if ratio is None else ratio * alg_bytes_per_launch,
                 "traffic_source": None if ratio is None else "profiles/step_kernel_traffic.csv: ncu dram bytes per algorithmic byte x this launch's algorithmic bytes",
                 "peak_source": peak_src, "kernel": kernel_name, "kernel_ms": kernel_ms, "kernel_launches_timed": kernel_n,
-                "kernel_share_of_step": kernel_ms / (ms / args.steps),
+                "kernel_share_of_step": kernel_ms / (ms_local / args.steps),
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch,
                 "whole_step_GBs": alg_bytes_per_launch / (ms * 1e-3 / args.steps) / 1e9,
                 "frac_of_8TBs_nominal": achieved / 8000.0}
