@@ -534,16 +534,14 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
 
 constexpr size_t ROWS_SMEM_MAX = 227 * 1024;
 
-// the instantiations: (storage type, nh_x, warps per group, groups, row blocks per octant chunk, early release);
-// the first one that fits is used unless UFS_DVM_ROWS picks another by index (timing experiments)
+// the instantiations: (storage type, nh_x, warps per group, groups, row blocks per octant chunk, early release).
+// Tried and slower on config 4 (fp32): two groups with early release (11.7 vs 9.6 ms on the quarter-size mesh), half
+// chunks per stage with five groups (14.8 ms), the same with early release (18.6 ms).
 struct RowsVariant { int storage, nhx, gw, ng, nq, early; };
 constexpr RowsVariant ROWS_VARIANTS[] = {
     {UFS_STORE_F32, 12, 5, 3, 1, 0},
     {UFS_STORE_F64, 12, 3, 5, 2, 0},
     {UFS_STORE_F64, 6, 2, 4, 1, 1},
-    {UFS_STORE_F32, 12, 5, 2, 1, 1},
-    {UFS_STORE_F32, 12, 3, 5, 2, 0},
-    {UFS_STORE_F32, 12, 3, 4, 2, 1},
 };
 constexpr int N_ROWS_VARIANTS = sizeof(ROWS_VARIANTS) / sizeof(ROWS_VARIANTS[0]);
 bool rows_variant_fits(const RowsVariant& rv, int storage, const VelLayout& v) {
@@ -552,10 +550,6 @@ bool rows_variant_fits(const RowsVariant& rv, int storage, const VelLayout& v) {
 }
 int rows_variant(int storage, const VelLayout& v) {
     if (!v.fast) return -1;
-    if (const char* e = std::getenv("UFS_DVM_ROWS")) {
-        const int i = std::atoi(e);
-        if (i >= 0 && i < N_ROWS_VARIANTS && rows_variant_fits(ROWS_VARIANTS[i], storage, v)) return i;
-    }
     for (int i = 0; i < N_ROWS_VARIANTS; i++)
         if (rows_variant_fits(ROWS_VARIANTS[i], storage, v)) return i;
     return -1;
@@ -594,6 +588,7 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan) 
     int ns = 16;
     while (ns >= 4 && rows_smem_bytes(elem, ns, slot, nw, tabn, nr) > ROWS_SMEM_MAX) ns--;
     if (ns < 4) return false;  // a 2:1 face needs four slots in flight at once
+    // UFS_DVM_NS / UFS_DVM_GRID: shallower ring / fewer CTAs, for the sensitivity runs quoted in profiles/
     if (const char* e = std::getenv("UFS_DVM_NS")) { const int f = std::atoi(e); if (f >= 4 && f < ns) ns = f; }
     *plan = base;
     plan->ring = 3;
@@ -614,9 +609,6 @@ cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p
         case 0: return launch_rows_t<float, 12, 5, 3, 1, false>(plan, p, st);
         case 1: return launch_rows_t<double, 12, 3, 5, 2, false>(plan, p, st);
         case 2: return launch_rows_t<double, 6, 2, 4, 1, true>(plan, p, st);
-        case 3: return launch_rows_t<float, 12, 5, 2, 1, true>(plan, p, st);
-        case 4: return launch_rows_t<float, 12, 3, 5, 2, false>(plan, p, st);
-        case 5: return launch_rows_t<float, 12, 3, 4, 2, true>(plan, p, st);
         default: return cudaErrorInvalidValue;
     }
 }
