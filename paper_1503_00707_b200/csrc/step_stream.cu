@@ -6,7 +6,7 @@
 // with, per cell,  H = sum_i m(xi_i) f_i  and  G[a][s] = sum_{i: sign(xi_a,i) = s} m(xi_i) |xi_a,i| f_i
 // (m = 1, xi, |xi|^2; 35 fp64 numbers).  These sums are produced for f^{n+1} by the pass that writes
 // f^{n+1}, so a step is
-//   k_prep   : per cell, rho* from the stored sums -> Newton for the discrete Maxwellian (the per-cell 5x5
+//   k_prep   : per cell (8 lanes each), rho* from the stored sums -> Newton for the discrete Maxwellian (the per-cell 5x5
 //              problem of PAPER.md:145-163, 179, separable form) -> factor table + dt*nu;   (~1 KB per cell)
 //   k_stream : per cell and velocity octant (sign group), four contiguous streams (own chunk
 //              + one upwind chunk per axis) arrive through a TMA ring (cp.async.bulk + mbarrier), and each
@@ -106,148 +106,178 @@ template <typename T> struct SeriesTol;   // residual below which one more (seri
 template <> struct SeriesTol<double> { static constexpr double value = 1e-7; };   // error after it ~1e-14
 template <> struct SeriesTol<float> { static constexpr double value = 1e-4; };    // ~1e-8 << fp32 storage rounding
 
-// Solve  w sum_i m(xi_i) exp(alpha . m(xi_i)) = rho with one warp.  exp(alpha.m) = A gx gy gz,
-// g_b[k] = exp(alpha_b xi_k + alpha_4 xi_k^2).  With the 1-D power sums P_b^r = sum_k xi_k^r g_b[k] the five
-// equations read  P_b^1/P_b^0 = u_b,  sum_b P_b^2/P_b^0 = rho_4/n,  A w Px^0 Py^0 Pz^0 = n: an arrow-shaped 4x4
-// Newton system (closed-form Schur complement) plus the amplitude.  Same root as a 5x5 Newton on alpha (the
-// solution is unique).  Stop: scaled residual <= 1e-13, or one more update after a residual <= SeriesTol (quadratic
-// convergence), that update applied to g through its series.  Lane k holds node k of every axis (nv <= 32).
+// Solve  w sum_i m(xi_i) exp(alpha . m(xi_i)) = rho, eight lanes per cell (four cells per warp).
+// exp(alpha.m) = A gx gy gz, g_b[k] = exp(alpha_b xi_k + alpha_4 xi_k^2).  With the 1-D power sums
+// P_b^r = sum_k xi_k^r g_b[k] the five equations read  P_b^1/P_b^0 = u_b,  sum_b P_b^2/P_b^0 = rho_4/n,
+// A w Px^0 Py^0 Pz^0 = n: an arrow-shaped 4x4 Newton system (closed-form Schur complement) plus the amplitude.  Same
+// root as a 5x5 Newton on alpha (the solution is unique).  Stop: scaled residual <= 1e-13, or one more update after a
+// residual <= SeriesTol (quadratic convergence), that update applied to g through its series.  Lane sl of a group holds
+// nodes sl, sl + 8, sl + 16, sl + 24 of every axis (nv <= 32).
+constexpr int PREP_NPL = 4;  // nodes per lane and axis
+__device__ __forceinline__ double group_sum(double v) {  // over the 8 lanes of a cell
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// four kinetic cells per warp
 template <typename T>
-__device__ __forceinline__ void newton_warp(const StepParams& p, const double (&rho)[5], int lane, T* tab) {
+__global__ void __launch_bounds__(256) k_prep(const StepParams p) {
+    const int lane = threadIdx.x & 31, sl = lane & 7;
+    const int cell_raw = (blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 4 + (lane >> 3);
+    const bool valid = cell_raw < p.n_kin;
+    const int cell = valid ? cell_raw : 0;
+    const int* rec = reinterpret_cast<const int*>(p.cells + cell);
+    const double* S = p.sums_in + (int64_t)cell * SUMS_STRIDE;
+    const int level = __ldg(rec + 24);
+    const double dth = p.dt * p.inv_len * (double)(1 << level);
+    // pair (d, k): net gain of moment k through direction d = 2*axis + side, in units of dt/h; a lane takes pairs
+    // sl, sl + 8, ... of the 30
+    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int idx = sl; idx < 30; idx += 8) {
+        const int d = idx / 5, k = idx % 5, a = d >> 1, side = d & 1, sin = 1 - side;
+        const int nsrc = __ldg(rec + d * 4 + 1) >= 0 ? 4 : 1;
+        double in = 0.0;
+        for (int j = 0; j < nsrc; j++) {
+            const int code = __ldg(rec + d * 4 + j);
+            const int kind = code >> SRC_SHIFT;
+            const int64_t idx2 = code & SRC_INDEX_MASK;
+            double v;
+            if (kind == SRC_SLAB) v = p.sums_in[idx2 * SUMS_STRIDE + g_index(a, sin, k)];
+            else if (kind == SRC_MIRROR) v = (k == 1 + a ? -1.0 : 1.0) * S[g_index(a, 1 - sin, k)];
+            else v = p.ghost_sums[(kind == SRC_TABLE ? idx2 : p.n_tables + idx2) * SUMS_STRIDE + g_index(a, sin, k)];
+            in += v;
+        }
+        const double contrib = (nsrc == 4 ? 0.25 : 1.0) * in - S[g_index(a, side, k)];
+#pragma unroll
+        for (int kk = 0; kk < 5; kk++) part[kk] += kk == k ? contrib : 0.0;
+    }
+    double rho[5];
+#pragma unroll
+    for (int k = 0; k < 5; k++) rho[k] = p.w * fma(dth, group_sum(part[k]), S[k]);
+
     const int nhp = nhp_of(p.nh);
     const double n = rho[0];
     const double inv_n = frcp(n);
     const double u[3] = {rho[1] * inv_n, rho[2] * inv_n, rho[3] * inv_n};
     const double e2 = rho[4] * inv_n;
     const double T0 = (e2 - (u[0] * u[0] + u[1] * u[1] + u[2] * u[2])) * (1.0 / 3.0);
-    const bool ok = (n > 0.0) && (T0 > 0.0);
+    bool ok = valid && (n > 0.0) && (T0 > 0.0);
     const double sqT = sqrt(ok ? T0 : 1.0);
     const double isc[4] = {frcp(sqT + fabs(u[0])), frcp(sqT + fabs(u[1])), frcp(sqT + fabs(u[2])), frcp(e2)};
     const double invT = frcp(T0);
     double al[4] = {u[0] * invT, u[1] * invT, u[2] * invT, -0.5 * invT};
-    double x[3], g[3] = {0.0, 0.0, 0.0}, P0f[3] = {1.0, 1.0, 1.0};
+    double g[3][PREP_NPL], P0f[3] = {1.0, 1.0, 1.0};
 #pragma unroll
-    for (int b = 0; b < 3; b++) x[b] = lane < p.nv[b] ? p.vel->xi[b][lane] : 0.0;
+    for (int b = 0; b < 3; b++)
+#pragma unroll
+        for (int j = 0; j < PREP_NPL; j++) g[b][j] = 0.0;
     bool done = false;
-    if (ok) {
-        for (int it = 0; it <= 50 && !done; it++) {
-            double P[3][5];
+    for (int it = 0; it <= 50; it++) {
+        const bool act = ok && !done;
+        if (!__any_sync(0xffffffffu, act)) break;
+        double P[3][5];
 #pragma unroll
-            for (int b = 0; b < 3; b++) {
-                g[b] = lane < p.nv[b] ? exp((al[b] + al[3] * x[b]) * x[b]) : 0.0;
-                double t = g[b];
+        for (int b = 0; b < 3; b++) {
+            double ps[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-                for (int r = 0; r < 5; r++) { P[b][r] = warp_sum(t); t *= x[b]; }
-            }
-            double m1[3], m2[3], i0[3], r[4];
-            r[3] = -e2;
+            for (int j = 0; j < PREP_NPL; j++) {
+                const int node = sl + 8 * j;
+                if (act && node < p.nv[b]) {
+                    const double x = p.vel->xi[b][node];
+                    double t = exp((al[b] + al[3] * x) * x);
+                    g[b][j] = t;
 #pragma unroll
-            for (int b = 0; b < 3; b++) {
-                i0[b] = frcp(P[b][0]);
-                m1[b] = P[b][1] * i0[b]; m2[b] = P[b][2] * i0[b];
-                r[b] = m1[b] - u[b];
-                r[3] += m2[b];
-            }
-            double res = 0.0;
-#pragma unroll
-            for (int k = 0; k < 4; k++) {
-                const double q = fabs(r[k]) * isc[k];
-                if (!(q <= res)) res = q;  // NaN propagates
-            }
-            if (res <= 1e-13) {
-#pragma unroll
-                for (int b = 0; b < 3; b++) P0f[b] = P[b][0];
-                done = true;
-                break;
-            }
-            if (!(res == res) || it == 50) break;
-            // arrow system: var_b d_b + c_b d_4 = -r_b ;  sum_b c_b d_b + dd d_4 = -r_4
-            double iv[3], cb[3], num = r[3], dd = 0.0, schur = 0.0;
-#pragma unroll
-            for (int b = 0; b < 3; b++) {
-                const double m3 = P[b][3] * i0[b], m4 = P[b][4] * i0[b];
-                iv[b] = frcp(m2[b] - m1[b] * m1[b]);
-                cb[b] = m3 - m1[b] * m2[b];
-                dd += m4 - m2[b] * m2[b];
-                schur += cb[b] * cb[b] * iv[b];
-                num -= cb[b] * r[b] * iv[b];
-            }
-            double dl[4];
-            dl[3] = -num * frcp(dd - schur);
-#pragma unroll
-            for (int b = 0; b < 3; b++) dl[b] = -(r[b] + cb[b] * dl[3]) * iv[b];
-#pragma unroll
-            for (int k = 0; k < 4; k++) al[k] += dl[k];
-            if (res <= SeriesTol<T>::value) {
-                // the update is small: apply it to g and to the zeroth power sums by expansion
-#pragma unroll
-                for (int b = 0; b < 3; b++) {
-                    const double z = (dl[b] + dl[3] * x[b]) * x[b];
-                    g[b] *= 1.0 + z * (1.0 + z * (0.5 + z * (1.0 / 6.0)));
-                    P0f[b] = P[b][0] + dl[b] * P[b][1] + dl[3] * P[b][2]
-                             + 0.5 * (dl[b] * dl[b] * P[b][2] + 2.0 * dl[b] * dl[3] * P[b][3] + dl[3] * dl[3] * P[b][4]);
+                    for (int r = 0; r < 5; r++) { ps[r] += t; t *= x; }
                 }
-                done = true;
             }
+#pragma unroll
+            for (int r = 0; r < 5; r++) P[b][r] = group_sum(ps[r]);
+        }
+        if (!act) continue;
+        double m1[3], m2[3], i0[3], r[4];
+        r[3] = -e2;
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            i0[b] = frcp(P[b][0]);
+            m1[b] = P[b][1] * i0[b]; m2[b] = P[b][2] * i0[b];
+            r[b] = m1[b] - u[b];
+            r[3] += m2[b];
+        }
+        double res = 0.0;
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            const double q = fabs(r[k]) * isc[k];
+            if (!(q <= res)) res = q;  // NaN propagates
+        }
+        if (res <= 1e-13) {
+#pragma unroll
+            for (int b = 0; b < 3; b++) P0f[b] = P[b][0];
+            done = true;
+            continue;
+        }
+        if (!(res == res) || it == 50) { ok = false; continue; }
+        // arrow system: var_b d_b + c_b d_4 = -r_b ;  sum_b c_b d_b + dd d_4 = -r_4
+        double iv[3], cb[3], num = r[3], dd = 0.0, schur = 0.0;
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            const double m3 = P[b][3] * i0[b], m4 = P[b][4] * i0[b];
+            iv[b] = frcp(m2[b] - m1[b] * m1[b]);
+            cb[b] = m3 - m1[b] * m2[b];
+            dd += m4 - m2[b] * m2[b];
+            schur += cb[b] * cb[b] * iv[b];
+            num -= cb[b] * r[b] * iv[b];
+        }
+        double dl[4];
+        dl[3] = -num * frcp(dd - schur);
+#pragma unroll
+        for (int b = 0; b < 3; b++) dl[b] = -(r[b] + cb[b] * dl[3]) * iv[b];
+#pragma unroll
+        for (int k = 0; k < 4; k++) al[k] += dl[k];
+        if (res <= SeriesTol<T>::value) {
+            // the update is small: apply it to g and to the zeroth power sums by expansion
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+#pragma unroll
+                for (int j = 0; j < PREP_NPL; j++) {
+                    const int node = sl + 8 * j;
+                    if (node < p.nv[b]) {
+                        const double x = p.vel->xi[b][node];
+                        const double z = (dl[b] + dl[3] * x) * x;
+                        g[b][j] *= 1.0 + z * (1.0 + z * (0.5 + z * (1.0 / 6.0)));
+                    }
+                }
+                P0f[b] = P[b][0] + dl[b] * P[b][1] + dl[3] * P[b][2]
+                         + 0.5 * (dl[b] * dl[b] * P[b][2] + 2.0 * dl[b] * dl[3] * P[b][3] + dl[3] * dl[3] * P[b][4]);
+            }
+            done = true;
         }
     }
+    if (!valid) return;
     double amp = 0.0, omega = 0.0;
     if (done) {
         amp = n * frcp(p.w * P0f[0] * P0f[1] * P0f[2]);
         // G9: nu = c_nu n T^(1-omega) / Kn (omega = 1/2: sqrt)
         const double Tp = (p.visc_exp == 0.5) ? sqT : pow(T0, 1.0 - p.visc_exp);
         omega = p.dt * p.nu_pref * n * Tp * p.inv_kn;
-    } else if (lane == 0) {
+    } else if (sl == 0) {
         atomicOr(p.flags, 1);  // no Maxwellian: f* passes through unchanged (UFS_DVM_ENEWTON)
     }
+    // table layout: stream_common.cuh
+    T* tab = reinterpret_cast<T*>(p.tabs) + (int64_t)cell * tabn_of(p.nh);
 #pragma unroll
     for (int b = 0; b < 3; b++) {
-        if (lane < p.nv[b]) {
-            const int s = lane >= p.nh[b] ? 1 : 0;
-            const int rk = s ? lane - p.nh[b] : p.nh[b] - 1 - lane;
-            tab[(2 * b + s) * nhp + rk] = done ? (T)(b == 2 ? g[b] * amp : g[b]) : T(0);
+#pragma unroll
+        for (int j = 0; j < PREP_NPL; j++) {
+            const int node = sl + 8 * j;
+            if (node < p.nv[b]) {
+                const int s = node >= p.nh[b] ? 1 : 0;
+                const int rk = s ? node - p.nh[b] : p.nh[b] - 1 - node;
+                tab[(2 * b + s) * nhp + rk] = done ? (T)(b == 2 ? g[b][j] * amp : g[b][j]) : T(0);
+            }
         }
     }
-    if (lane == 0) tab[6 * nhp] = (T)omega;
-}
-
-// one warp per kinetic cell
-template <typename T>
-__global__ void __launch_bounds__(256) k_prep(const StepParams p) {
-    const int lane = threadIdx.x & 31;
-    const int cell = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (cell >= p.n_kin) return;
-    const int* rec = reinterpret_cast<const int*>(p.cells + cell);
-    const double* S = p.sums_in + (int64_t)cell * SUMS_STRIDE;
-    const int level = __ldg(rec + 24);
-    const double dth = p.dt * p.inv_len * (double)(1 << level);
-    // lane (d, k): net gain of moment k through direction d = 2*axis + side, in units of dt/h
-    double contrib = 0.0;
-    if (lane < 30) {
-        const int d = lane / 5, k = lane % 5, a = d >> 1, side = d & 1, sin = 1 - side;
-        const int nsrc = __ldg(rec + d * 4 + 1) >= 0 ? 4 : 1;
-        double in = 0.0;
-        for (int j = 0; j < nsrc; j++) {
-            const int code = __ldg(rec + d * 4 + j);
-            const int kind = code >> SRC_SHIFT;
-            const int64_t idx = code & SRC_INDEX_MASK;
-            double v;
-            if (kind == SRC_SLAB) v = p.sums_in[idx * SUMS_STRIDE + g_index(a, sin, k)];
-            else if (kind == SRC_MIRROR) v = (k == 1 + a ? -1.0 : 1.0) * S[g_index(a, 1 - sin, k)];
-            else v = p.ghost_sums[(kind == SRC_TABLE ? idx : p.n_tables + idx) * SUMS_STRIDE + g_index(a, sin, k)];
-            in += v;
-        }
-        contrib = (nsrc == 4 ? 0.25 : 1.0) * in - S[g_index(a, side, k)];
-    }
-    double rho[5];
-#pragma unroll
-    for (int k = 0; k < 5; k++) {
-        double t = 0.0;
-#pragma unroll
-        for (int d = 0; d < 6; d++) t += __shfl_sync(0xffffffffu, contrib, d * 5 + k);
-        rho[k] = p.w * fma(dth, t, S[k]);
-    }
-    newton_warp<T>(p, rho, lane, reinterpret_cast<T*>(p.tabs) + (int64_t)cell * tabn_of(p.nh));
+    if (sl == 0) tab[6 * nhp] = (T)omega;
 }
 
 // moments of the current f from its stored sums: mom[5][n_kin] = (n, n u, E = rho_4 / 2)
@@ -691,7 +721,7 @@ template <typename T, int PIECES>
 cudaError_t launch_stream_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
     if (p.collide) {
         const int wpb = 8;
-        k_prep<T><<<(p.n_kin + wpb - 1) / wpb, wpb * 32, 0, st>>>(p);
+        k_prep<T><<<(p.n_kin + 4 * wpb - 1) / (4 * wpb), wpb * 32, 0, st>>>(p);
     }
     auto k = k_stream<T, STREAM_NCW, PIECES>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
@@ -741,8 +771,9 @@ bool stream_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan
 cudaError_t launch_prep(int storage, const StepParams& p, cudaStream_t st) {
     if (p.n_kin == 0 || !p.collide) return cudaSuccess;
     const int wpb = 8;
-    if (storage == UFS_STORE_F32) k_prep<float><<<(p.n_kin + wpb - 1) / wpb, wpb * 32, 0, st>>>(p);
-    else k_prep<double><<<(p.n_kin + wpb - 1) / wpb, wpb * 32, 0, st>>>(p);
+    const int blocks = (p.n_kin + 4 * wpb - 1) / (4 * wpb);  // four cells per warp
+    if (storage == UFS_STORE_F32) k_prep<float><<<blocks, wpb * 32, 0, st>>>(p);
+    else k_prep<double><<<blocks, wpb * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
