@@ -122,7 +122,7 @@ __device__ __forceinline__ double group_sum(double v) {  // over the 8 lanes of 
 
 // four kinetic cells per warp
 template <typename T>
-__global__ void __launch_bounds__(256) k_prep(const StepParams p) {
+__global__ void __launch_bounds__(256, 3) k_prep(const StepParams p) {
     const int lane = threadIdx.x & 31, sl = lane & 7;
     const int cell_raw = (blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 4 + (lane >> 3);
     const bool valid = cell_raw < p.n_kin;
