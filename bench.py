@@ -6,7 +6,7 @@ Workload (N=1): the configuration the north-star target is stated on -- the ~1.0
 octree with a 24^3 velocity grid, fp32 storage, fp64 moment accumulation (BASELINE.json configs[3],
 SURVEY.md 8(d) row 4); both f buffers (2 x 55.8 GB) resident in HBM.  Synthetic, seeded inputs.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3|config5]
     python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
 
 N > 1 runs N independent replicas (the path is one GPU by the north star).
@@ -38,6 +38,8 @@ def make_case(workload: str):
         return inputs.config2()
     if workload == "config3":
         return inputs.config3(lmax=8)
+    if workload == "config5":
+        return inputs.config5(lmax=8)
     raise SystemExit(f"unknown workload {workload}")
 
 
