@@ -361,14 +361,18 @@ int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
     for (int64_t s = 0; s < m.n_kin; s++) {
         CellRec& r = m.recs[s];
         r.level = d.level[m.cell_of_slab[s]];
-        bool simple = true, nofluid = true;
+        bool simple = true, nofluid = true, ringfluid = true;
         for (int dd = 0; dd < 6; dd++) {
             const int c = cnt[(size_t)s * 6 + dd];
             if (c != 1 && c != 4) ok = false;
             if (c != 1) simple = false;
-            for (int k = 0; k < c; k++) if ((r.src[dd][k] >> SRC_SHIFT) == SRC_FLUID) simple = nofluid = false;
+            for (int k = 0; k < c; k++)
+                if ((r.src[dd][k] >> SRC_SHIFT) == SRC_FLUID) {
+                    simple = nofluid = false;
+                    if (c != 1) ringfluid = false;  // a fluid leaf among four finer neighbours: plain gather path
+                }
         }
-        r.flags = (simple ? CELL_SIMPLE : 0) | (nofluid ? CELL_NOFLUID : 0);
+        r.flags = (simple ? CELL_SIMPLE : 0) | (nofluid ? CELL_NOFLUID : 0) | (!nofluid && ringfluid ? CELL_RINGFLUID : 0);
         m.n_simple += simple;
     }
     if (!ok) { err = "internal: a kinetic cell has a direction with neither 1 nor 4 sources"; return UFS_DVM_EMESH; }

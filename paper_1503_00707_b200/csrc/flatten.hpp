@@ -34,12 +34,13 @@ inline int32_t src_code(SrcKind k, int64_t idx) { return (int32_t)((k << SRC_SHI
 struct CellRec {
     int32_t src[6][4];
     int32_t level;
-    int32_t flags;  // bit 0: every direction has exactly one source and none is SRC_FLUID; bit 1: no source is SRC_FLUID
+    int32_t flags;  // bit 0: every direction has exactly one source and none is SRC_FLUID; bit 1: no source is SRC_FLUID; bit 2: CELL_RINGFLUID
     int32_t pad[6];
 };
 static_assert(sizeof(CellRec) == 128, "CellRec must be 128 bytes");
 constexpr int32_t CELL_SIMPLE = 1;
 constexpr int32_t CELL_NOFLUID = 2;
+constexpr int32_t CELL_RINGFLUID = 4;  // some source is SRC_FLUID, and every direction with one has that source alone
 
 constexpr int NV_MAX = 64;  // per-axis node limit (tables live in shared memory)
 

@@ -147,12 +147,38 @@ __device__ __forceinline__ void row_finish(const StepParams& p, const RowCtx<T, 
     }
 }
 
+// Upwind values of a kinetic/fluid face (reading G13): the pointwise Maxwellian of the fluid leaf's frozen
+// moments, from its separable factors; `code` is the source code of the direction, j the 16-byte vector of the row.
+template <typename T>
+__device__ __forceinline__ void fluid_vec(const StepParams& p, int code, int o, int j, int ry, int rz, T (&v)[V16<T>::N]) {
+    constexpr int VEC = V16<T>::N;
+    const FluidGhost* g = p.fluid + (code & SRC_INDEX_MASK);
+    const int kz = ((o >> 2) & 1) ? p.nh[2] + rz : p.nh[2] - 1 - rz;
+    const int ky = ((o >> 1) & 1) ? p.nh[1] + ry : p.nh[1] - 1 - ry;
+    const double b = g->amp * g->g[2][kz] * g->g[1][ky];
+#pragma unroll
+    for (int i = 0; i < VEC; i++) {
+        const int kx = (o & 1) ? p.nh[0] + j * VEC + i : p.nh[0] - 1 - j * VEC - i;
+        v[i] = (T)(b * g->g[0][kx]);
+    }
+}
+// what row_from_ring needs to know about the fluid streams of a stage (fm = 0: none)
+struct FluidStreams { int fm, o, ry, rz; const int* rec; };
+template <typename T>
+__device__ __forceinline__ void apply_fluid(const StepParams& p, const FluidStreams& fs, int j, T (&X)[V16<T>::N], T (&Y)[V16<T>::N],
+                                            T (&Z)[V16<T>::N]) {
+    if (fs.fm & 1) fluid_vec<T>(p, fs.rec[(1 - (fs.o & 1)) * 4], fs.o, j, fs.ry, fs.rz, X);
+    if (fs.fm & 2) fluid_vec<T>(p, fs.rec[(2 + 1 - ((fs.o >> 1) & 1)) * 4], fs.o, j, fs.ry, fs.rz, Y);
+    if (fs.fm & 4) fluid_vec<T>(p, fs.rec[(4 + 1 - ((fs.o >> 2) & 1)) * 4], fs.o, j, fs.ry, fs.rz, Z);
+}
+
 // One row from the four streams of a ring slot.  EARLY: the whole row is read into registers first and the slot is
 // handed back to the producer before the arithmetic (the ring then holds data in flight, not data in use).
-template <typename T, int NHX, int NQ, bool EARLY>
+// FLUID: streams whose source is a fluid leaf are not in the slot; they are computed (apply_fluid).
+template <typename T, int NHX, int NQ, bool EARLY, bool FLUID>
 __device__ __forceinline__ void row_from_ring(const StepParams& p, const RowCtx<T, NQ>& rc, int q, T wb, const T* st, int pe,
-                                              const T* gxrow, T* gdst, bool active, int lane, uint32_t empty_bar, double& s0,
-                                              double& s1, double& s2, double& s3) {
+                                              const T* gxrow, T* gdst, bool active, int lane, uint32_t empty_bar,
+                                              const FluidStreams& fs, double& s0, double& s1, double& s2, double& s3) {
     constexpr int VEC = V16<T>::N, RV = NHX / VEC;
     if (EARLY) {
         T own[RV][VEC], X[RV][VEC], Y[RV][VEC], Z[RV][VEC];
@@ -163,6 +189,7 @@ __device__ __forceinline__ void row_from_ring(const StepParams& p, const RowCtx<
                 lds16(st + pe + j * VEC, X[j]);
                 lds16(st + 2 * pe + j * VEC, Y[j]);
                 lds16(st + 3 * pe + j * VEC, Z[j]);
+                if (FLUID && fs.fm) apply_fluid<T>(p, fs, j, X[j], Y[j], Z[j]);
             }
         }
         __syncwarp();
@@ -180,6 +207,7 @@ __device__ __forceinline__ void row_from_ring(const StepParams& p, const RowCtx<
                 lds16(st + pe + j * VEC, X);
                 lds16(st + 2 * pe + j * VEC, Y);
                 lds16(st + 3 * pe + j * VEC, Z);
+                if (FLUID && fs.fm) apply_fluid<T>(p, fs, j, X, Y, Z);
                 row_finish<T, NHX, NQ>(p, rc, q, wb, j, own, X, Y, Z, gxrow, gdst, s0, s1, s2, s3);
             }
         }
@@ -207,7 +235,7 @@ __device__ __forceinline__ void row_from_gather(const StepParams& p, const RowCt
     }
 }
 
-template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY>
+template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY, bool FLUID>
 __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams p) {
     constexpr int VEC = V16<T>::N, RV = NHX / VEC, NW = NG * GW;
     constexpr int MAXST = (8 * NQ + NG - 1) / NG;  // stages of one cell that can fall to one group
@@ -267,7 +295,7 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
             __syncwarp();
         };
         // issue octants [o0, o1) of cell `cur`; rec = this lane's word of the cell record, masks = 3 bits per octant
-        auto issue = [&](int cur, int rec, int masks, int o0, int o1) {
+        auto issue = [&](int cur, int rec, int masks, int fmasks, int o0, int o1) {
             // lane (o,t): stream t of octant o -- t = 0 own chunk, t = 1..3 the upwind chunk on axis t-1
             const int a = t_l > 0 ? t_l - 1 : 0;
             const int dir = 2 * a + (1 - ((o_l >> a) & 1));
@@ -282,8 +310,10 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                 const int xdir = lane < 3 ? 2 * lane + (1 - ((o >> lane) & 1)) : 0;
 #pragma unroll
                 for (int q = 0; q < NQ; q++) {
-                    arm(slot_bytes);
-                    if (o_l == o)
+                    // streams from a fluid leaf are not copied (the consumers compute them)
+                    const int fm = FLUID ? (fmasks >> (3 * o)) & 7 : 0;
+                    arm(slot_bytes - (uint32_t)__popc(fm) * piece_bytes);
+                    if (o_l == o && !(t_l > 0 && ((fm >> (t_l - 1)) & 1)))
                         sbulk_g2s(sb + s.ring + slot * slot_bytes + t_l * piece_bytes, ptr + (size_t)q * pe, piece_bytes,
                                   sb + s.full + 8u * slot);
                     skip(1);
@@ -325,7 +355,7 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
             // enough that the atomic and the record load (two dependent global round trips) hide behind the copies.
             const int nxt_raw = fetch_async();
             const int level = __shfl_sync(0xffffffffu, rec, 24), flags = __shfl_sync(0xffffffffu, rec, 25);
-            const bool ringable = (flags & CELL_NOFLUID) != 0;
+            const bool ringable = (flags & CELL_NOFLUID) != 0 || (FLUID && (flags & CELL_RINGFLUID) != 0);
             // bit d: direction d has four (finer) sources instead of one
             int four = 0;
 #pragma unroll
@@ -339,8 +369,22 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
 #pragma unroll
             for (int d = 1; d < 8; d <<= 1) { masks |= __shfl_xor_sync(0xffffffffu, masks, d); mbits |= __shfl_xor_sync(0xffffffffu, mbits, d); }
             masks = __shfl_sync(0xffffffffu, masks, 0); mbits = __shfl_sync(0xffffffffu, mbits, 0);
+            // axes whose upwind source is a fluid leaf (computed by the consumers, not copied), 3 bits per octant
+            int fmasks = 0;
+            if (FLUID && (flags & CELL_RINGFLUID)) {
+                int myf = 0;
+#pragma unroll
+                for (int b = 0; b < 3; b++) {
+                    const int code = __shfl_sync(0xffffffffu, rec, (2 * b + (1 - ((lane >> b) & 1))) * 4);
+                    myf |= ((code >> SRC_SHIFT) == SRC_FLUID ? 1 : 0) << b;
+                }
+                fmasks = lane < 8 ? myf << (3 * lane) : 0;
+#pragma unroll
+                for (int d = 1; d < 8; d <<= 1) fmasks |= __shfl_xor_sync(0xffffffffu, fmasks, d);
+                fmasks = __shfl_sync(0xffffffffu, fmasks, 0);
+            }
             hdr[HDR_REC + lane] = rec;
-            if (lane == 0) { hdr[0] = cur; hdr[1] = level; hdr[2] = ringable ? CK_RING : CK_GATHER; hdr[3] = mbits; hdr[4] = masks; }
+            if (lane == 0) { hdr[0] = cur; hdr[1] = level; hdr[2] = ringable ? CK_RING : CK_GATHER; hdr[3] = mbits; hdr[4] = masks; hdr[5] = fmasks; }
             __syncwarp();
             if (lane == 0) {
                 const uint32_t cf = sb + s.cfull + 8u * cs;
@@ -354,7 +398,7 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
             }
             const int nxt = __shfl_sync(0xffffffffu, nxt_raw, 0);
             const int nrec = load_rec(nxt);  // in flight while this cell's copies are issued
-            if (ringable) issue(cur, rec, masks, 0, 8);
+            if (ringable) issue(cur, rec, masks, fmasks, 0, 8);
             cur = nxt;
             rec = nrec;
         }
@@ -389,6 +433,7 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
         const double dth = p.dt * p.inv_len * (double)(1 << h0.y);  // dt / h
         const int mbits = h0.w;  // 1 bit per octant: it has a 2:1 upwind face
         const int masks = *reinterpret_cast<const int*>(smem_raw + hdr + 16);  // 3 bits per octant: on which axes
+        const int fmasks = FLUID ? *reinterpret_cast<const int*>(smem_raw + hdr + 20) : 0;  // ... the source is a fluid leaf
         RowCtx<T, NQ> rc;
         rc.omega = p.collide ? tab[6 * nhp] : T(0);
         const double om1 = 1.0 - (double)rc.omega;
@@ -478,7 +523,11 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                     }
                     // a slot written with ordinary stores: order them before the bulk copy that refills it
                     if (mask) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    row_from_ring<T, NHX, NQ, EARLY>(p, rc, q, wb, st, pe, gxrow, gdst, active, lane, sb + s.empty + 8u * slot,
+                    FluidStreams fs;
+                    fs.fm = FLUID ? (fmasks >> (3 * o)) & 7 : 0;
+                    fs.o = o; fs.ry = ry[q]; fs.rz = rz[q];
+                    fs.rec = reinterpret_cast<const int*>(smem_raw + hdr + HDR_REC * 4);
+                    row_from_ring<T, NHX, NQ, EARLY, FLUID>(p, rc, q, wb, st, pe, gxrow, gdst, active, lane, sb + s.empty + 8u * slot, fs,
                                                      S[i][0], S[i][1], S[i][2], S[i][3]);
                 } else if (active) {
                     row_from_gather<T, NHX, NQ>(p, rc, q, wb, o, CH, q * NRQ + r, ry[q], rz[q], reinterpret_cast<const int*>(p.cells + cell),
@@ -555,9 +604,9 @@ int rows_variant(int storage, const VelLayout& v) {
     return -1;
 }
 
-template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY>
-cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
-    auto k = k_rows<T, NHX, GW, NG, NQ, EARLY>;
+template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY, bool FLUID>
+cudaError_t launch_rows_t2(const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
+    auto k = k_rows<T, NHX, GW, NG, NQ, EARLY, FLUID>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_kin < plan.grid ? p.n_kin : plan.grid;
@@ -565,6 +614,12 @@ cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStrea
     k<<<grid, (NG * GW + 1) * 32, plan.smem_bytes, st>>>(p);
     if (plan.ev1) cudaEventRecord(plan.ev1, st);
     return cudaGetLastError();
+}
+
+template <typename T, int NHX, int GW, int NG, int NQ, bool EARLY>
+cudaError_t launch_rows_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
+    return p.fluid ? launch_rows_t2<T, NHX, GW, NG, NQ, EARLY, true>(plan, p, st)
+                   : launch_rows_t2<T, NHX, GW, NG, NQ, EARLY, false>(plan, p, st);
 }
 
 }  // namespace
@@ -606,6 +661,7 @@ cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p
     cudaError_t e = launch_prep(storage, p, st);
     if (e != cudaSuccess) return e;
     switch (plan.ncw) {
+        // (meshes with fluid leaves get the instantiation that computes fluid streams; the others keep the leaner code)
         case 0: return launch_rows_t<float, 12, 5, 3, 1, false>(plan, p, st);
         case 1: return launch_rows_t<double, 12, 3, 5, 2, false>(plan, p, st);
         case 2: return launch_rows_t<double, 6, 2, 4, 1, true>(plan, p, st);
