@@ -99,6 +99,25 @@ def test_generic_and_odd_velocity_grids(nv, vmin, vmax):
     assert info["fast"] == sym_even
 
 
+@pytest.mark.parametrize("nv,storage,kernel", [((16, 16, 16), inputs.STORE_F64, "k_stream"),
+                                               ((16, 8, 8), inputs.STORE_F32, "k_stream"),
+                                               ((12, 12, 12), inputs.STORE_F64, "k_rows"),
+                                               ((24, 12, 8), inputs.STORE_F32, "k_rows"),
+                                               ((12, 12, 12), inputs.STORE_F32, "k_step_fast")])
+def test_kernel_selection_and_parity_on_other_even_grids(nv, storage, kernel):
+    """Every streaming kernel and its fallbacks: k_rows needs nh_x in {6, 12} (fp32: 12), k_stream a whole number of
+    16-byte vectors per x run, the one-CTA-per-cell kernel takes the rest.  2:1 faces and specular walls included."""
+    lv, ijk = random_tree(np.random.default_rng(11), 1, 3, (True, False, True), 0.3)
+    bc = (inputs.BC_PERIODIC, inputs.BC_PERIODIC, inputs.BC_SPECULAR, inputs.BC_SPECULAR, inputs.BC_PERIODIC, inputs.BC_PERIODIC)
+    case = periodic_case(lv, ijk, nv=nv, kn=0.2, bc=bc)
+    rng = np.random.default_rng(3)
+    f0 = inputs.maxwellian_canonical(case, case.prim0) * (1 + 0.2 * rng.uniform(-1, 1, (case.n_leaves, case.Nv)))
+    st = B.DvmStepper(case, storage=storage)
+    assert B.ufs_dvm_kernel_name(st.h) == kernel
+    st.close()
+    check(case, 3, TOL[storage], storage=storage, f0=f0)
+
+
 def test_specular_box_with_odd_grid_generic_path():
     lv, ijk = inputs.build_tree(2, 2, {}, P)
     case = periodic_case(lv, ijk, nv=(5, 5, 5), bc=(inputs.BC_SPECULAR,) * 6, kn=0.3)
