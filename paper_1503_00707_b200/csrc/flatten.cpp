@@ -373,6 +373,14 @@ int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
                 }
         }
         r.flags = (simple ? CELL_SIMPLE : 0) | (nofluid ? CELL_NOFLUID : 0) | (!nofluid && ringfluid ? CELL_RINGFLUID : 0);
+        // per velocity octant: which upwind directions (xi_a > 0: the low side) bring four sources / a fluid source
+        r.masks = r.fmasks = 0;
+        for (int o = 0; o < 8; o++)
+            for (int a = 0; a < 3; a++) {
+                const int dd = 2 * a + (1 - ((o >> a) & 1));
+                if (cnt[(size_t)s * 6 + dd] == 4) r.masks |= 1 << (3 * o + a);
+                else if ((r.src[dd][0] >> SRC_SHIFT) == SRC_FLUID) r.fmasks |= 1 << (3 * o + a);
+            }
         m.n_simple += simple;
     }
     if (!ok) { err = "internal: a kinetic cell has a direction with neither 1 nor 4 sources"; return UFS_DVM_EMESH; }

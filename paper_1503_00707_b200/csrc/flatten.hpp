@@ -35,7 +35,9 @@ struct CellRec {
     int32_t src[6][4];
     int32_t level;
     int32_t flags;  // bit 0: every direction has exactly one source and none is SRC_FLUID; bit 1: no source is SRC_FLUID; bit 2: CELL_RINGFLUID
-    int32_t pad[6];
+    int32_t masks;   // 3 bits per velocity octant o (bit a): the upwind face of o on axis a has four finer sources
+    int32_t fmasks;  // 3 bits per octant: the upwind source on axis a is a fluid leaf (single source)
+    int32_t pad[4];
 };
 static_assert(sizeof(CellRec) == 128, "CellRec must be 128 bytes");
 constexpr int32_t CELL_SIMPLE = 1;

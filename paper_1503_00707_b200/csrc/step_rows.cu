@@ -356,33 +356,11 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
             const int nxt_raw = fetch_async();
             const int level = __shfl_sync(0xffffffffu, rec, 24), flags = __shfl_sync(0xffffffffu, rec, 25);
             const bool ringable = (flags & CELL_NOFLUID) != 0 || (FLUID && (flags & CELL_RINGFLUID) != 0);
-            // bit d: direction d has four (finer) sources instead of one
-            int four = 0;
-#pragma unroll
-            for (int d = 0; d < 6; d++) four |= (__shfl_sync(0xffffffffu, rec, d * 4 + 1) >= 0 ? 1 : 0) << d;
-            // axes whose upwind face has four finer sources, for the octant of this lane (lanes 0..7)
-            int mymask = 0;
-#pragma unroll
-            for (int b = 0; b < 3; b++) mymask |= ((four >> (2 * b + (1 - ((lane >> b) & 1)))) & 1) << b;
-            if (!ringable || lane >= 8) mymask = 0;
-            int masks = mymask << (3 * (lane & 7)), mbits = (mymask ? 1 : 0) << (lane & 7);
-#pragma unroll
-            for (int d = 1; d < 8; d <<= 1) { masks |= __shfl_xor_sync(0xffffffffu, masks, d); mbits |= __shfl_xor_sync(0xffffffffu, mbits, d); }
-            masks = __shfl_sync(0xffffffffu, masks, 0); mbits = __shfl_sync(0xffffffffu, mbits, 0);
-            // axes whose upwind source is a fluid leaf (computed by the consumers, not copied), 3 bits per octant
-            int fmasks = 0;
-            if (FLUID && (flags & CELL_RINGFLUID)) {
-                int myf = 0;
-#pragma unroll
-                for (int b = 0; b < 3; b++) {
-                    const int code = __shfl_sync(0xffffffffu, rec, (2 * b + (1 - ((lane >> b) & 1))) * 4);
-                    myf |= ((code >> SRC_SHIFT) == SRC_FLUID ? 1 : 0) << b;
-                }
-                fmasks = lane < 8 ? myf << (3 * lane) : 0;
-#pragma unroll
-                for (int d = 1; d < 8; d <<= 1) fmasks |= __shfl_xor_sync(0xffffffffu, fmasks, d);
-                fmasks = __shfl_sync(0xffffffffu, fmasks, 0);
-            }
+            // which octants have a 2:1 upwind face, on which axes; which upwind sources are fluid leaves (computed by the
+            // consumers, not copied): 3 bits per octant, precomputed by the flattener
+            const int masks = ringable ? __shfl_sync(0xffffffffu, rec, 26) : 0;
+            const int fmasks = FLUID && ringable ? __shfl_sync(0xffffffffu, rec, 27) : 0;
+            const int mbits = (int)(__ballot_sync(0xffffffffu, lane < 8 && ((masks >> (3 * lane)) & 7) != 0) & 0xffu);
             hdr[HDR_REC + lane] = rec;
             if (lane == 0) { hdr[0] = cur; hdr[1] = level; hdr[2] = ringable ? CK_RING : CK_GATHER; hdr[3] = mbits; hdr[4] = masks; hdr[5] = fmasks; }
             __syncwarp();
