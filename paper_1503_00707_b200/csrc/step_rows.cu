@@ -387,13 +387,12 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
     const int g = warp / GW;
     const int r = (warp % GW) * 32 + lane;  // row inside a stage
     const bool active = r < NRQ;
-    double ay[NQ], az[NQ];
+    // (|xi_y|, |xi_z| of the row are re-read from shared memory where needed: registers are what this kernel is short of)
+    const double2* ayz = reinterpret_cast<const double2*>(smem_raw + s.ayz);
     int ry[NQ], rz[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; q++) {
         const int row = active ? q * NRQ + r : 0;
-        const double2 yz = reinterpret_cast<const double2*>(smem_raw + s.ayz)[row];
-        ay[q] = yz.x; az[q] = yz.y;
         ry[q] = row % p.nh[1]; rz[q] = row / p.nh[1];
     }
     const uint32_t inv_ns = (65536u + (uint32_t)NS - 1u) / (uint32_t)NS;  // x / NS = (x * inv_ns) >> 16 for x < 128
@@ -418,24 +417,22 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
         rc.sx = (T)(om1 * dth);
 #pragma unroll
         for (int q = 0; q < NQ; q++) {
-            rc.base[q] = (T)(om1 * (1.0 - dth * (ay[q] + az[q])));
-            rc.cy[q] = (T)(om1 * dth * ay[q]);
-            rc.cz[q] = (T)(om1 * dth * az[q]);
+            const double2 yz = ayz[active ? q * NRQ + r : 0];
+            rc.base[q] = (T)(om1 * (1.0 - dth * (yz.x + yz.y)));
+            rc.cy[q] = (T)(om1 * dth * yz.x);
+            rc.cz[q] = (T)(om1 * dth * yz.y);
         }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)cell * p.Nv;
         // this group's stages of the cell: first, first + NG, ...  (stage = octant * NQ + row block)
         int first = g - turn0;
         if (first < 0) first += NG;
         double S[MAXST][4];  // the row sums of this thread's stages (registers: the loops over them are unrolled)
-        int so[MAXST];
 #pragma unroll
         for (int i = 0; i < MAXST; i++) {
             const int stg = first + i * NG;
-            so[i] = -1;
             S[i][0] = S[i][1] = S[i][2] = S[i][3] = 0.0;
             if (stg < 8 * NQ) {
                 const int o = stg / NQ, q = stg % NQ;
-                so[i] = stg;
                 const int mask = (masks >> (3 * o)) & 7;
                 const T* gxrow = tab + (o & 1) * nhp;
                 T* const gdst = gcell + (int64_t)o * CH + (int64_t)(q * NRQ + r) * NHX;
@@ -529,9 +526,10 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
         for (int i = 0; i < 35; i++) acc[i] = 0.0;
 #pragma unroll
         for (int i = 0; i < MAXST; i++) {
-            if (so[i] >= 0 && active) {
-                const int q = so[i] % NQ;
-                fold_row_rt(so[i] / NQ, S[i][0], S[i][1], S[i][2], S[i][3], NQ > 1 && q ? ay[NQ - 1] : ay[0], NQ > 1 && q ? az[NQ - 1] : az[0], acc);
+            const int stg = first + i * NG;
+            if (stg < 8 * NQ && active) {
+                const double2 yz = ayz[(stg % NQ) * NRQ + r];
+                fold_row_rt(stg / NQ, S[i][0], S[i][1], S[i][2], S[i][3], yz.x, yz.y, acc);
             }
         }
         warp_store_sums(acc, reinterpret_cast<double*>(smem_raw + s.red) + ((size_t)cs * NW + warp) * SUMS_STRIDE, lane);
