@@ -43,6 +43,7 @@ struct StepParams {
     // row kernel (step_rows.cu): |xi_x| of the x ranks and its powers (uniform operands, constant bank)
     double xpow[3][16];         // [r-1][rank] = |xi_x|^r, r = 1..3
     float xf[16];               // |xi_x| in fp32
+    uint32_t smap[12];          // row kernel: its shared-memory map (byte offsets), computed by the launcher
 };
 
 constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used)

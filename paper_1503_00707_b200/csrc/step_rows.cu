@@ -250,7 +250,10 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
     const uint32_t tab_bytes = (uint32_t)tabn * (uint32_t)sizeof(T);
     const uint32_t cell_bytes = (uint32_t)rows_cell_bytes(sizeof(T), tabn);
     const int NS = p.ring_stages;
-    const RowsSmem s = rows_map(sizeof(T), NS, slot_bytes, NW, tabn, NR);
+    // the shared-memory map comes with the kernel parameters (constant bank): nothing of it has to live in registers
+    RowsSmem s;
+    s.ring = p.smap[0]; s.cells = p.smap[1]; s.red = p.smap[2]; s.ayz = p.smap[3]; s.full = p.smap[4]; s.empty = p.smap[5];
+    s.cfull = p.smap[6]; s.cempty = p.smap[7]; s.cnt = p.smap[8]; s.issued = p.smap[9]; s.total = p.smap[10];
     const uint32_t sb = smem_u32(smem_raw);  // shared-space address of the map's origin
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
@@ -586,8 +589,15 @@ cudaError_t launch_rows_t2(const StepLaunch& plan, const StepParams& p, cudaStre
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_kin < plan.grid ? p.n_kin : plan.grid;
+    StepParams q = p;
+    {
+        const int nr = p.nh[1] * p.nh[2];
+        const RowsSmem m = rows_map(sizeof(T), p.ring_stages, (size_t)4 * (nr / NQ) * NHX * sizeof(T), NG * GW, tabn_of(p.nh), nr);
+        const uint32_t v[11] = {m.ring, m.cells, m.red, m.ayz, m.full, m.empty, m.cfull, m.cempty, m.cnt, m.issued, m.total};
+        for (int i = 0; i < 11; i++) q.smap[i] = v[i];
+    }
     if (plan.ev0) cudaEventRecord(plan.ev0, st);
-    k<<<grid, (NG * GW + 1) * 32, plan.smem_bytes, st>>>(p);
+    k<<<grid, (NG * GW + 1) * 32, plan.smem_bytes, st>>>(q);
     if (plan.ev1) cudaEventRecord(plan.ev1, st);
     return cudaGetLastError();
 }
