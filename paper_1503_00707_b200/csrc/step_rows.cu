@@ -440,7 +440,15 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                 const T* gxrow = tab + (o & 1) * nhp;
                 T* const gdst = gcell + (int64_t)o * CH + (int64_t)(q * NRQ + r) * NHX;
                 T wb = T(0);
-                if (p.collide) wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rz[q]] * tab[(2 + ((o >> 1) & 1)) * nhp + ry[q]]);
+                // this stage's row block: picked by selects, not by indexing (NQ <= 2; indexing would put the arrays in
+                // local memory)
+                RowCtx<T, 1> rq;
+                rq.base[0] = NQ > 1 && q ? rc.base[NQ - 1] : rc.base[0];
+                rq.cy[0] = NQ > 1 && q ? rc.cy[NQ - 1] : rc.cy[0];
+                rq.cz[0] = NQ > 1 && q ? rc.cz[NQ - 1] : rc.cz[0];
+                rq.sx = rc.sx; rq.omega = rc.omega;
+                const int ryq = NQ > 1 && q ? ry[NQ - 1] : ry[0], rzq = NQ > 1 && q ? rz[NQ - 1] : rz[0];
+                if (p.collide) wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rzq] * tab[(2 + ((o >> 1) & 1)) * nhp + ryq]);
                 if (kind == CK_RING) {
                     // ring slots taken by the stages before this one: one each, four where the octant has a 2:1 face
                     const int before = stg + 3 * (NQ * __popc(mbits & ((1 << o) - 1)) + (mask ? q : 0));
@@ -503,12 +511,12 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                     if (mask) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     FluidStreams fs;
                     fs.fm = FLUID ? (fmasks >> (3 * o)) & 7 : 0;
-                    fs.o = o; fs.ry = ry[q]; fs.rz = rz[q];
+                    fs.o = o; fs.ry = ryq; fs.rz = rzq;
                     fs.rec = reinterpret_cast<const int*>(smem_raw + hdr + HDR_REC * 4);
-                    row_from_ring<T, NHX, NQ, EARLY, FLUID>(p, rc, q, wb, st, pe, gxrow, gdst, active, lane, sb + s.empty + 8u * slot, fs,
+                    row_from_ring<T, NHX, 1, EARLY, FLUID>(p, rq, 0, wb, st, pe, gxrow, gdst, active, lane, sb + s.empty + 8u * slot, fs,
                                                      S[i][0], S[i][1], S[i][2], S[i][3]);
                 } else if (active) {
-                    row_from_gather<T, NHX, NQ>(p, rc, q, wb, o, CH, q * NRQ + r, ry[q], rz[q], reinterpret_cast<const int*>(p.cells + cell),
+                    row_from_gather<T, NHX, 1>(p, rq, 0, wb, o, CH, q * NRQ + r, ryq, rzq, reinterpret_cast<const int*>(p.cells + cell),
                                                 fin, cell, gxrow, gdst, S[i][0], S[i][1], S[i][2], S[i][3]);
                 }
             }
