@@ -418,12 +418,12 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
         rc.omega = p.collide ? tab[6 * nhp] : T(0);
         const double om1 = 1.0 - (double)rc.omega;
         rc.sx = (T)(om1 * dth);
-#pragma unroll
-        for (int q = 0; q < NQ; q++) {
-            const double2 yz = ayz[active ? q * NRQ + r : 0];
-            rc.base[q] = (T)(om1 * (1.0 - dth * (yz.x + yz.y)));
-            rc.cy[q] = (T)(om1 * dth * yz.x);
-            rc.cz[q] = (T)(om1 * dth * yz.y);
+        const double omd = om1 * dth;
+        if (NQ == 1) {  // one row per thread and cell: its coefficients are formed once per cell (else per stage, below)
+            const double2 yz = ayz[active ? r : 0];
+            rc.base[0] = (T)(om1 - omd * (yz.x + yz.y));
+            rc.cy[0] = (T)(omd * yz.x);
+            rc.cz[0] = (T)(omd * yz.y);
         }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)cell * p.Nv;
         // this group's stages of the cell: first, first + NG, ...  (stage = octant * NQ + row block)
@@ -443,9 +443,14 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                 // this stage's row block: picked by selects, not by indexing (NQ <= 2; indexing would put the arrays in
                 // local memory)
                 RowCtx<T, 1> rq;
-                rq.base[0] = NQ > 1 && q ? rc.base[NQ - 1] : rc.base[0];
-                rq.cy[0] = NQ > 1 && q ? rc.cy[NQ - 1] : rc.cy[0];
-                rq.cz[0] = NQ > 1 && q ? rc.cz[NQ - 1] : rc.cz[0];
+                if (NQ == 1) {
+                    rq.base[0] = rc.base[0]; rq.cy[0] = rc.cy[0]; rq.cz[0] = rc.cz[0];
+                } else {  // several row blocks: form the row's coefficients here rather than keep NQ sets in registers
+                    const double2 yz = ayz[active ? q * NRQ + r : 0];
+                    rq.base[0] = (T)(om1 - omd * (yz.x + yz.y));
+                    rq.cy[0] = (T)(omd * yz.x);
+                    rq.cz[0] = (T)(omd * yz.y);
+                }
                 rq.sx = rc.sx; rq.omega = rc.omega;
                 const int ryq = NQ > 1 && q ? ry[NQ - 1] : ry[0], rzq = NQ > 1 && q ? rz[NQ - 1] : rz[0];
                 if (p.collide) wb = rc.omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rzq] * tab[(2 + ((o >> 1) & 1)) * nhp + ryq]);
