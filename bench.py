@@ -68,34 +68,49 @@ def ncu_traffic_ratio(workload: str):
 
 
 def oracle_sample(case, n_sample: int):
-    """A bounded sample of the workload for the CPU oracle: the window made of the first n_sample
-    leaves in Morton order (missing neighbours at the window edge become zero-gradient ghosts)."""
-    from paper_1503_00707_b200 import binding as B
-    from paper_1503_00707_b200 import harness
-    desc, keep = B.make_desc(case)
-    h = B.ufs_dvm_create_host(desc)
-    _, cell_of_slab, _ = B.ufs_dvm_layout(h, case.Nv)
-    B.ufs_dvm_destroy(h)
-    ids = np.sort(cell_of_slab[:n_sample])
-    return harness.sub_case(case, ids, case.name + "_sample")
+    """A bounded sample of the workload for the CPU oracle: the window made of the first n_sample kinetic leaves in
+    Morton order plus the non-kinetic leaves among them (missing neighbours at the window edge become zero-gradient
+    ghosts).  Computed here with numpy: this leg never loads the CUDA library."""
+    from paper_1503_00707_b200 import inputs
+    order = inputs.morton_order(case.level, case.ijk)
+    kin_pos = np.nonzero(case.kind[order] == inputs.CELL_KINETIC)[0]
+    last = kin_pos[min(n_sample, kin_pos.size) - 1]
+    return inputs.sub_case(case, np.sort(order[:last + 1]), case.name + "_sample")
 
 
-def time_oracle(case, n_sample: int, steps: int, warmup: int):
+def time_oracle(case, n_sample: int, steps: int, warmup: int, one_thread_leaves: int = 0):
+    """The oracle as it stands (fp64, OpenMP over cells) on a Morton window of the workload: all cores, `steps` steps
+    (>= 3 by BASELINE.md section 3); optionally also with 1 thread on a smaller window."""
     from oracle import dvm_oracle
     from paper_1503_00707_b200 import inputs
-    sub = oracle_sample(case, n_sample)
-    o = dvm_oracle.Oracle(sub, window=True)
-    f = inputs.initial_f(sub)
-    for _ in range(warmup):
-        f = o.step(f, case.dt)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        f = o.step(f, case.dt)
-    t = time.perf_counter() - t0
-    units = o.n_kinetic * sub.Nv * steps
-    return {"value": units / t, "unit": UNIT, "cores": dvm_oracle.threads(), "kind": "oracle",
-            "sample": f"window of the first {o.n_kinetic} Morton-ordered leaves of {case.name}, {steps} steps "
-                      f"(fp64, OpenMP over cells)", "seconds": t}, t / steps
+
+    def run(n_leaves, n_threads, k, w):
+        sub = oracle_sample(case, n_leaves)
+        dvm_oracle.set_threads(n_threads)
+        o = dvm_oracle.Oracle(sub, window=True)     # neighbour-table build: outside the timed region
+        f = inputs.initial_f(sub)
+        for _ in range(w):
+            f = o.step(f, case.dt)
+        t0 = time.perf_counter()
+        for _ in range(k):
+            f = o.step(f, case.dt)
+        t = time.perf_counter() - t0
+        return o.n_kinetic * sub.Nv * k / t, t, o.n_kinetic
+
+    cores = os.cpu_count() or dvm_oracle.threads()
+    cores = min(cores, dvm_oracle.threads()) if dvm_oracle.threads() > 1 else cores
+    steps = max(3, steps)
+    value, t, n_kin = run(n_sample, cores, steps, warmup)
+    out = {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"window of the first {n_kin} Morton-ordered kinetic leaves of {case.name}, {steps} steps "
+                     f"(fp64, OpenMP over cells, {cores} threads)", "seconds": t}
+    if one_thread_leaves:
+        v1, t1, n1 = run(one_thread_leaves, 1, steps, 0)
+        out["value_1_thread"] = v1
+        out["sample_1_thread"] = f"first {n1} Morton-ordered kinetic leaves, {steps} steps, 1 thread"
+        out["seconds"] = t + t1
+        dvm_oracle.set_threads(cores)
+    return out, t / steps
 
 
 def run_reference(args):
@@ -104,12 +119,13 @@ def run_reference(args):
         return
     case = make_case(args.workload)
     n_sample = args.oracle_leaves or 4096
-    base, ms = time_oracle(case, n_sample, max(1, args.steps), args.warmup)
+    base, sec = time_oracle(case, n_sample, args.steps, args.warmup, one_thread_leaves=max(64, n_sample // 16))
+    keys = ("value", "unit", "cores", "kind", "sample", "value_1_thread", "sample_1_thread")
     line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms * 1e3, "higher_is_better": True,
+            "steps": max(3, args.steps), "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(case, args),
-            "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": {k: base[k] for k in keys if k in base},
             "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -256,8 +272,10 @@ def main():
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         st.close(); del st
         torch.cuda.empty_cache()
-        base, _ = time_oracle(case, args.oracle_leaves or 16384, 2, 0)
-        line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        n_or = args.oracle_leaves or 16384
+        base, _ = time_oracle(case, n_or, 3, 0, one_thread_leaves=n_or // 16)
+        keys = ("value", "unit", "cores", "kind", "sample", "value_1_thread", "sample_1_thread")
+        line["cpu_baseline"] = {k: base[k] for k in keys if k in base}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

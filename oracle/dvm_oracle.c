@@ -524,3 +524,12 @@ int oracle_dvm_threads(void) {
     return 1;
 #endif
 }
+
+/* timing aid (bench.py: the oracle with 1 thread and with all cores); no effect on any result */
+void oracle_dvm_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}

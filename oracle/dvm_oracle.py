@@ -146,3 +146,8 @@ class Oracle:
 
 def threads():
     return int(lib().oracle_dvm_threads())
+
+
+def set_threads(n: int):
+    """OpenMP threads of the following oracle calls (bench.py times the oracle with 1 thread and with all cores)."""
+    lib().oracle_dvm_set_threads(int(n))

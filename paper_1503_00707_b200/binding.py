@@ -244,27 +244,34 @@ class DvmStepper:
         assert f_rows.shape == (self.n_kinetic, self.Nv)
         cur = ufs_dvm_current(self.h)
         chunk = max(1, (1 << 28) // (self.Nv * 8))
-        for s0 in range(0, self.n_kinetic, chunk):
-            rows = self.row_of_slab[s0:s0 + chunk]
-            part = f_rows[rows][:, self.vel_of_slot]
-            self.f[cur][s0:s0 + chunk].copy_(torch.from_numpy(np.ascontiguousarray(part)).to(self.dtype))
+        slot_t = torch.as_tensor(self.vel_of_slot.astype(np.int64), device=self.device)
+        with torch.cuda.stream(self.stream):     # the copies must be ordered with the handle's stream
+            for s0 in range(0, self.n_kinetic, chunk):
+                rows = self.row_of_slab[s0:s0 + chunk]
+                part = torch.from_numpy(np.ascontiguousarray(f_rows[rows])).to(self.device)
+                self.f[cur][s0:s0 + chunk].copy_(part.index_select(1, slot_t).to(self.dtype))
         ufs_dvm_f_changed(self.h)
 
     def read_canonical(self, slabs: Optional[np.ndarray] = None) -> np.ndarray:
-        """Current f as float64 [rows, Nv] in canonical order.  With `slabs`, only those slabs, in the
-        order given (rows are then slabs, not Case rows)."""
+        """Current f as float64 [rows, Nv] in canonical velocity order.  With `slabs`, only those slabs, in the
+        order given (rows are then slabs, not Case rows).  The slot permutation is applied on the device."""
         torch = self.torch
         cur = ufs_dvm_current(self.h)
-        torch.cuda.synchronize(self.device)
         inv = np.empty(self.Nv, np.int64); inv[self.vel_of_slot] = np.arange(self.Nv)
-        if slabs is not None:
-            idx = torch.as_tensor(np.asarray(slabs, np.int64), device=self.device)
-            return self.f[cur][idx].double().cpu().numpy()[:, inv]
-        out = np.empty((self.n_kinetic, self.Nv))
+        inv_t = torch.as_tensor(inv, device=self.device)
         chunk = max(1, (1 << 28) // (self.Nv * 8))
-        for s0 in range(0, self.n_kinetic, chunk):
-            part = self.f[cur][s0:s0 + chunk].double().cpu().numpy()[:, inv]
-            out[self.row_of_slab[s0:s0 + chunk]] = part
+        with torch.cuda.stream(self.stream):
+            if slabs is not None:
+                slabs = np.asarray(slabs, np.int64)
+                out = np.empty((slabs.size, self.Nv))
+                for s0 in range(0, slabs.size, chunk):
+                    idx = torch.as_tensor(slabs[s0:s0 + chunk], device=self.device)
+                    out[s0:s0 + chunk] = self.f[cur].index_select(0, idx).index_select(1, inv_t).double().cpu().numpy()
+                return out
+            out = np.empty((self.n_kinetic, self.Nv))
+            for s0 in range(0, self.n_kinetic, chunk):
+                part = self.f[cur][s0:s0 + chunk].index_select(1, inv_t).double().cpu().numpy()
+                out[self.row_of_slab[s0:s0 + chunk]] = part
         return out
 
     def step(self, dt: float, nsteps: int = 1):

@@ -10,6 +10,7 @@ from typing import Optional
 import numpy as np
 
 from . import binding as B
+from . import inputs as _inputs
 from .inputs import STORE_F32, Case
 
 
@@ -26,42 +27,21 @@ def fill_initial_f_device(st: "B.DvmStepper", case: Case, chunk_slabs: int = 204
     kx, ky, kz = vel % nvx, (vel // nvx) % nvy, vel // (nvx * nvy)
     xs, ys, zs = (torch.as_tensor(case.xi_nodes(a), device=dev) for a in range(3))
     prim = torch.as_tensor(case.prim0[st.cell_of_slab], device=dev)            # [n_kin, 5] in slab order
-    for s0 in range(0, st.n_kinetic, chunk_slabs):
-        p = prim[s0:s0 + chunk_slabs]
-        n, ux, uy, uz, T = (p[:, c:c + 1] for c in range(5))
-        ex = torch.exp(-(xs[None, :] - ux) ** 2 / (2 * T))
-        ey = torch.exp(-(ys[None, :] - uy) ** 2 / (2 * T))
-        ez = torch.exp(-(zs[None, :] - uz) ** 2 / (2 * T))
-        a = n / (2 * np.pi * T) ** 1.5
-        f = a * ez[:, kz] * ey[:, ky] * ex[:, kx]
-        st.f[cur][s0:s0 + chunk_slabs].copy_(f.to(st.dtype))
+    with torch.cuda.stream(st.stream):           # ordered with the handle's stream
+        for s0 in range(0, st.n_kinetic, chunk_slabs):
+            p = prim[s0:s0 + chunk_slabs]
+            n, ux, uy, uz, T = (p[:, c:c + 1] for c in range(5))
+            ex = torch.exp(-(xs[None, :] - ux) ** 2 / (2 * T))
+            ey = torch.exp(-(ys[None, :] - uy) ** 2 / (2 * T))
+            ez = torch.exp(-(zs[None, :] - uz) ** 2 / (2 * T))
+            a = n / (2 * np.pi * T) ** 1.5
+            f = a * ez[:, kz] * ey[:, ky] * ex[:, kx]
+            st.f[cur][s0:s0 + chunk_slabs].copy_(f.to(st.dtype))
     B.ufs_dvm_f_changed(st.h)
 
 
-def window_leaves(case: Case, centre_leaf: int, rings: int, neighbours_of) -> np.ndarray:
-    """Leaf ids within `rings` face-rings of `centre_leaf` (breadth-first over face neighbours)."""
-    keep = {int(centre_leaf)}
-    front = [int(centre_leaf)]
-    for _ in range(rings):
-        nxt = []
-        for j in neighbours_of(front).tolist():
-            if j not in keep:
-                keep.add(j); nxt.append(j)
-        front = nxt
-        if not front:
-            break
-    return np.array(sorted(keep), dtype=np.int64)
-
-
-def sub_case(case: Case, leaf_ids: np.ndarray, name: Optional[str] = None) -> Case:
-    """The Case restricted to some leaves (a window of the mesh; the oracle takes it with window=True)."""
-    import copy
-    sub = copy.copy(case)
-    sub.level, sub.ijk, sub.kind = case.level[leaf_ids].copy(), case.ijk[leaf_ids].copy(), case.kind[leaf_ids].copy()
-    sub.prim0 = case.prim0[leaf_ids].copy()
-    sub.fluid_moments = None if case.fluid_moments is None else case.fluid_moments[leaf_ids].copy()
-    sub.name = name or (case.name + "_window")
-    return sub
+# mesh slicing lives with the problem descriptions (no arithmetic of the method): re-exported for the tests
+window_leaves, sub_case = _inputs.window_leaves, _inputs.sub_case
 
 
 class ClockSampler:

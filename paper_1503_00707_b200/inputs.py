@@ -382,23 +382,39 @@ def small(config: int) -> Case:
     raise ValueError(config)
 
 
-def window_case(case: Case, centre_leaf: int, rings: int, neighbours_of) -> tuple:
-    """Sub-problem for the windowed check at full size: all leaves within `rings`
-    face-rings of `centre_leaf`.  `neighbours_of(leaf_ids) -> leaf ids` must return the face
-    neighbours (a pure mesh query supplied by the caller).  Returns (leaf ids kept, sub-Case)."""
+def window_leaves(case: Case, centre_leaf: int, rings: int, neighbours_of) -> np.ndarray:
+    """Leaf ids within `rings` face-rings of `centre_leaf` (breadth-first over face neighbours)."""
     keep = {int(centre_leaf)}
-    front = np.array([centre_leaf])
+    front = [int(centre_leaf)]
     for _ in range(rings):
-        nb = np.unique(neighbours_of(front))
-        nb = np.array([x for x in nb.tolist() if x not in keep], dtype=np.int64)
-        keep.update(nb.tolist())
-        front = nb
-        if front.size == 0:
+        nxt = []
+        for j in neighbours_of(front).tolist():
+            if j not in keep:
+                keep.add(j); nxt.append(j)
+        front = nxt
+        if not front:
             break
-    ids = np.array(sorted(keep), dtype=np.int64)
-    sub = Case(**{**case.__dict__})
-    sub.level, sub.ijk, sub.kind = case.level[ids].copy(), case.ijk[ids].copy(), case.kind[ids].copy()
-    sub.prim0 = case.prim0[ids].copy()
-    sub.fluid_moments = None if case.fluid_moments is None else case.fluid_moments[ids].copy()
-    sub.name = case.name + "_window"
-    return ids, sub
+    return np.array(sorted(keep), dtype=np.int64)
+
+
+def sub_case(case: Case, leaf_ids: np.ndarray, name: Optional[str] = None) -> Case:
+    """The Case restricted to some leaves (a window of the mesh; the oracle takes it with window=True)."""
+    import copy
+    sub = copy.copy(case)
+    sub.level, sub.ijk, sub.kind = case.level[leaf_ids].copy(), case.ijk[leaf_ids].copy(), case.kind[leaf_ids].copy()
+    sub.prim0 = case.prim0[leaf_ids].copy()
+    sub.fluid_moments = None if case.fluid_moments is None else case.fluid_moments[leaf_ids].copy()
+    sub.name = name or (case.name + "_window")
+    return sub
+
+
+def morton_order(level: np.ndarray, ijk: np.ndarray) -> np.ndarray:
+    """Leaf ids in N-order (Morton; reading G15: depth-first, child index x + 2y + 4z)."""
+    level = np.asarray(level).astype(np.int64)
+    lmax = int(level.max())
+    xyz = np.asarray(ijk).astype(np.int64) << (lmax - level)[:, None]
+    key = np.zeros(level.shape[0], np.int64)
+    for b in range(lmax):
+        for a in range(3):
+            key |= ((xyz[:, a] >> b) & 1) << (3 * b + a)
+    return np.argsort(key * 32 + level, kind="stable")

@@ -63,3 +63,36 @@ def np_moments(case, f):
     w = np.prod([(case.vmax[a] - case.vmin[a]) / case.nv[a] for a in range(3)])
     m = np.stack([np.ones_like(X), X, Y, Z, X * X + Y * Y + Z * Z])
     return w * (f @ m.T)
+
+
+def moment_scales(m_ref, eps_storage=2.3e-16):
+    """Denominators of the relative L-infinity error (G17) of the five moment fields [5, n].  The three momentum
+    components are one vector field: they are scaled by the largest norm of the momentum vector.  Only a momentum
+    field that is zero to round-off (no larger than 1e3 storage roundings of n * sqrt(R T0)) falls back to max n."""
+    m_ref = np.asarray(m_ref)
+    n_max = float(np.abs(m_ref[0]).max())
+    p_max = float(np.sqrt((m_ref[1:4] ** 2).sum(axis=0)).max())
+    if p_max <= 1e3 * eps_storage * n_max:
+        p_max = n_max
+    return [n_max, p_max, p_max, p_max, float(np.abs(m_ref[4]).max())]
+
+
+def assert_moments_close(m_gpu, m_ref, tol, eps_storage=2.3e-16, what=""):
+    scales = moment_scales(m_ref, eps_storage)
+    for a in range(5):
+        err = float(np.abs(np.asarray(m_gpu[a]) - np.asarray(m_ref[a])).max()) / scales[a]
+        assert err <= tol, f"{what} moment {a}: {err:.3e} > {tol:g}"
+
+
+def gpu_field_error(st, f_ref, chunk_slabs=2048):
+    """max|f_gpu - f_ref| and max|f_ref| over the whole field, read from the device slab chunk by slab chunk
+    (f_ref rows are Case kinetic rows, canonical velocity order)."""
+    dmax = rmax = 0.0
+    for s0 in range(0, st.n_kinetic, chunk_slabs):
+        slabs = np.arange(s0, min(s0 + chunk_slabs, st.n_kinetic))
+        got = st.read_canonical(slabs)
+        ref = f_ref[st.row_of_slab[slabs]]
+        assert np.all(np.isfinite(got))
+        dmax = max(dmax, float(np.abs(got - ref).max()))
+        rmax = max(rmax, float(np.abs(ref).max()))
+    return dmax, rmax

@@ -9,7 +9,7 @@ import pytest
 from oracle.dvm_oracle import Oracle
 from paper_1503_00707_b200 import binding as B
 from paper_1503_00707_b200 import inputs
-from tests.helpers import periodic_case, random_tree, rel_linf
+from tests.helpers import assert_moments_close, periodic_case, random_tree, rel_linf
 
 pytestmark = pytest.mark.gpu
 TOL = {inputs.STORE_F64: 1e-12, inputs.STORE_F32: 2e-5}
@@ -42,12 +42,11 @@ def check(case, nsteps, tol, **kw):
     assert np.all(np.isfinite(f_gpu))
     err_f = rel_linf(f_gpu, f_ref)
     assert err_f <= tol, f"f: {err_f:.3e}"
-    for a in range(5):
-        scale = np.abs(m_ref[a]).max()
-        if a in (1, 2, 3):   # a momentum component may vanish (noise only): scale by n * velocity unit sqrt(R T0)
-            scale = max(scale, np.abs(m_ref[0]).max())
-        err = np.abs(m_gpu[a] - m_ref[a]).max() / scale
-        assert err <= tol, f"moment {a}: {err:.3e}"
+    storage = kw.get("storage")
+    storage = case.storage if storage is None else storage
+    # moments: never tighter than the stated tolerance of the storage type (a tiny momentum field, e.g. noise only,
+    # carries the summation round-off of n * sqrt(R T0) on a scale of its own norm)
+    assert_moments_close(m_gpu, m_ref, max(tol, TOL[storage]), eps_storage=6e-8 if storage == inputs.STORE_F32 else 2.3e-16)
     return info
 
 
