@@ -75,17 +75,21 @@ typedef struct {
  * The buffers are recorded, not read: before the first step the caller fills f_dev[0] with f at t = 0 in
  * the library's layout, slab s = leaf cell_of_slab[s], slot t = velocity node vel_of_slot[t]
  * (ufs_dvm_layout).  Validates the tree (EMESH) and the grid (EINVAL: specular sides and SOLID leaves
- * need vmin = -vmax on the wall-normal axis; Nv * sizeof(element) must fit the on-chip slab buffer). */
+ * need vmin = -vmax on the wall-normal axis; where only the one-CTA-per-cell kernels apply, Nv * sizeof(element)
+ * must fit their on-chip slab buffer). */
 int ufs_dvm_create(const ufs_dvm_desc *desc, void *f_dev[2], void *cuda_stream, ufs_dvm_t *out);
 
 /* Same flattening and validation without touching CUDA: the handle answers ufs_dvm_layout,
  * ufs_dvm_faces, ufs_dvm_boundary_faces and ufs_dvm_destroy; device calls return EINVAL. */
 int ufs_dvm_create_host(const ufs_dvm_desc *desc, ufs_dvm_t *out);
 
-/* Enqueue nsteps explicit steps of size dt (transport -> moments -> discrete Maxwellian -> BGK
- * relaxation, one fused kernel per step).  f ping-pongs between the two buffers.  The environment
- * variable UFS_DVM_KERNEL=cell (read by ufs_dvm_create) selects the one-CTA-per-cell kernels even where
- * the persistent ring kernel applies. */
+/* Enqueue nsteps explicit steps of size dt (transport -> moments -> discrete Maxwellian -> BGK relaxation).
+ * f ping-pongs between the two buffers.  A step is two launches: k_prep (per cell: the moments of f* from the carried
+ * velocity sums, Newton for the discrete Maxwellian) and the streaming pass that reads f once and writes f once
+ * (k_tiles where the velocity grid has 12 positive nodes on x and whole 48-row blocks, e.g. 24^3; else k_rows,
+ * k_stream, or the one-CTA-per-cell kernels, which need no k_prep); one more pass (the velocity sums of f) before
+ * the first step and after ufs_dvm_f_changed.  The environment variable UFS_DVM_KERNEL = rows | stream | cell (read at
+ * creation) forces the later kernels of that list (A/B timing, tests of the fallbacks). */
 int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps);
 
 /* Enqueue the moments of the current f: mom_dev is DEVICE memory, [5][n_kinetic] doubles in slab order:
@@ -132,6 +136,17 @@ int ufs_dvm_boundary_faces(ufs_dvm_t h, int64_t *n_faces, int64_t *cell, int8_t 
 int ufs_dvm_run_host(ufs_dvm_t h, const void *f_host_in, void *f_host_out, double *mom_dev_scratch,
                      double *mom_host, double dt, int nsteps);
 
+/* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
+ * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
+ * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes (bit 31: inflow ghost table, else
+ * slab * 8 + octant); cellidx[n_tiles][8][8][16] bytes = per octant and cell: [0] own piece, [1] flags (bit a: axis a
+ * has four finer sources, bit 3: a fluid source), [4 + 4a + k] piece of source k on axis a (0xFF unused, 0xFE fluid
+ * leaf); fluid[n_tiles][8][24] = fluid ghost of source k of direction d at [d*4+k] (only if the mesh has FLUID
+ * leaves); fluid_leaf[*n_fluid_ghosts] = leaf of each fluid ghost.  First-order form of the per-cell, per-sign-group
+ * stencil records of PAPER.md:113-115, deduplicated per tile. */
+int ufs_dvm_tiles(ufs_dvm_t h, int64_t *n_tiles, int32_t *pmax, int32_t *hdr, uint32_t *pieces, uint8_t *cellidx,
+                  int32_t *fluid, int64_t *n_fluid_ghosts, int64_t *fluid_leaf);
+
 /* Number of kernels this handle has launched so far (step + moments kernels). */
 int64_t ufs_dvm_launch_count(ufs_dvm_t h);
 
@@ -146,8 +161,9 @@ int ufs_dvm_kernel_ms(ufs_dvm_t h, double *mean_ms, int32_t *n_launches);
  * elements, and 1 if the octant fast path is used (0 = generic per-slot path).  HOST outputs. */
 int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t *threads, int32_t *smem_bytes, int32_t *vec, int32_t *fast);
 
-/* Name of the step kernel this handle launches: "k_step_ring" (persistent TMA ring kernel),
- * "k_step_fast" (one CTA per cell, octant layout) or "k_step_generic" (any velocity grid).  Never NULL. */
+/* Name of the streaming kernel this handle launches: "k_tiles" (persistent, tiles of up to eight slabs share their
+ * upwind chunks on chip), "k_rows" / "k_stream" (persistent, one cell at a time), "k_step_fast" (one CTA per cell,
+ * octant layout) or "k_step_generic" (any velocity grid).  Never NULL. */
 const char *ufs_dvm_kernel_name(ufs_dvm_t h);
 
 /* Message of the last error on this handle (valid until the next call on it); never NULL. */

@@ -20,7 +20,7 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
-           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms"]
+           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -60,6 +60,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp]
         L.ufs_dvm_boundary_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
         L.ufs_dvm_run_host.argtypes = [vp, vp, vp, vp, vp, C.c_double, C.c_int]
+        L.ufs_dvm_tiles.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int32), vp, vp, vp, vp, C.POINTER(C.c_int64), vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
@@ -180,6 +181,21 @@ def ufs_dvm_boundary_faces(h):
     _check(h, lib().ufs_dvm_boundary_faces(h, C.byref(n), cell.ctypes.data, axis.ctypes.data, side.ctypes.data,
                                            area.ctypes.data, kind.ctypes.data, state.ctypes.data))
     return cell, axis, side, area, kind, state
+
+
+def ufs_dvm_tiles(h) -> dict:
+    """The flattener's tile records (see include/ufs_dvm.h); empty arrays if the handle uses another kernel."""
+    n, pmax, ng = C.c_int64(), C.c_int32(), C.c_int64()
+    _check(h, lib().ufs_dvm_tiles(h, C.byref(n), C.byref(pmax), None, None, None, None, C.byref(ng), None))
+    nt, pm = int(n.value), int(pmax.value)
+    hdr = np.zeros((nt, 8), np.int32); pieces = np.zeros((nt, 8, max(pm, 1)), np.uint32)
+    cellidx = np.zeros((nt, 8, 8, 16), np.uint8); fluid = np.full((nt, 8, 24), -1, np.int32)
+    fluid_leaf = np.zeros(int(ng.value), np.int64)
+    _check(h, lib().ufs_dvm_tiles(h, C.byref(n), C.byref(pmax), hdr.ctypes.data, pieces.ctypes.data if pm else None,
+                                  cellidx.ctypes.data, fluid.ctypes.data, C.byref(ng), fluid_leaf.ctypes.data))
+    return {"n_tiles": nt, "pmax": pm, "s0": hdr[:, 0].copy(), "nc": hdr[:, 1].copy(),
+            "np": hdr[:, 2:4].copy().view(np.uint8).reshape(nt, 8), "level": hdr[:, 4:6].copy().view(np.uint8).reshape(nt, 8),
+            "pieces": pieces, "cellidx": cellidx, "fluid": fluid, "fluid_leaf": fluid_leaf}
 
 
 def ufs_dvm_run_host(h, f_host_in_ptr: int, f_host_out_ptr: Optional[int], mom_dev_ptr: int, mom_host_ptr: int,

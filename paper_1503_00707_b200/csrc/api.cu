@@ -32,6 +32,11 @@ struct ufs_dvm_s {
     double* d_sums[2] = {nullptr, nullptr};
     double* d_ghost_sums = nullptr;
     void* d_tabs = nullptr;
+    // tile kernel: the flattener's tile records
+    TileHdr* d_tile_hdr = nullptr;
+    uint32_t* d_tile_pieces = nullptr;
+    uint8_t* d_tile_cellidx = nullptr;
+    int32_t* d_tile_fluid = nullptr;
     bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
     StepLaunch plan{};
@@ -100,6 +105,12 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.ghost_sums = h->d_ghost_sums;
     p.tabs = h->d_tabs;
     p.n_tables = h->mesh.n_tables;
+    p.tile_hdr = h->d_tile_hdr;
+    p.tile_pieces = h->d_tile_pieces;
+    p.tile_cellidx = h->d_tile_cellidx;
+    p.tile_fluid = h->d_tile_fluid;
+    p.n_tiles = (int32_t)h->mesh.tiles.size();
+    p.tile_pmax = h->mesh.tile_pmax;
     if (v.fast) {
         for (int r = 0; r < v.nh[0] && r < 16; r++) {
             const double x = v.xi[0][v.nh[0] + r];
@@ -149,6 +160,27 @@ int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out) {
     const char* why = "";
     int rc = step_plan(h->storage, h->mesh.vel, &h->plan, &why);
     if (rc) return fail(h, rc, why);
+    // Kernel choice: the tile kernel (step_tiles.cu) where the velocity grid fits it, else the streaming step with one
+    // row per thread (step_rows.cu), else one vector per thread (step_stream.cu), else one CTA per cell (kernels.cu).
+    // UFS_DVM_KERNEL = rows | stream | cell forces the later ones (A/B timing, tests of the fallbacks).  The grid size
+    // (one CTA per SM) is filled in by ufs_dvm_create once the device is known.
+    const char* force = std::getenv("UFS_DVM_KERNEL");
+    const bool want_cell = force && std::strcmp(force, "cell") == 0;
+    const bool want_vec = force && std::strcmp(force, "stream") == 0;
+    const bool want_rows = force && std::strcmp(force, "rows") == 0;
+    if (!want_cell) {
+        int pmax = 0;
+        StepLaunch cand{};
+        if (!want_vec && !want_rows && tiles_plan(h->storage, h->mesh.vel, 1, &cand, &pmax)) {
+            h->plan = cand;
+            try {
+                build_tiles(h->mesh, pmax);
+            } catch (const std::bad_alloc&) {
+                return fail(h, UFS_DVM_ENOMEM, "out of host memory while building the tile records");
+            }
+        } else if (!want_vec && rows_plan(h->storage, h->mesh.vel, 1, &cand)) h->plan = cand;
+        else if (stream_plan(h->storage, h->mesh.vel, 1, &cand)) h->plan = cand;
+    }
     return UFS_DVM_OK;
 }
 
@@ -194,20 +226,17 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     CU(cudaMemsetAsync(h->d_flags, 0, 4, h->stream), "clear flags");
     CU(cudaMalloc(reinterpret_cast<void**>(&h->d_counter), 8), "allocate cell counters");
     CU(cudaMemsetAsync(h->d_counter, 0, 8, h->stream), "clear cell counters");
-    // kernel choice: the persistent TMA ring kernel where the velocity grid fits it, else one CTA per cell
-    // (UFS_DVM_KERNEL=cell forces the latter: A/B timing and tests)
-    // Kernel choice: the streaming step (one row per thread, else one vector per thread) where the velocity grid fits
-    // it, else one CTA per cell.  UFS_DVM_KERNEL = stream | cell forces the older variants (A/B timing, tests).
-    const char* force = std::getenv("UFS_DVM_KERNEL");
-    const bool want_cell = force && std::strcmp(force, "cell") == 0;
-    const bool want_vec = force && std::strcmp(force, "stream") == 0;
-    if (!want_cell) {
+    if (h->plan.ring >= 2) {
         int dev = 0, sms = 0;
         CU(cudaGetDevice(&dev), "get device");
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
-        StepLaunch cand{};
-        if (!want_vec && rows_plan(h->storage, v, sms, &cand)) h->plan = cand;
-        else if (stream_plan(h->storage, v, sms, &cand)) h->plan = cand;
+        h->plan.grid = sms;   // persistent kernels: one CTA per SM
+    }
+    if (h->plan.ring == 4) {
+        if ((rc = upload(h, &h->d_tile_hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr), "upload tile headers"))) return rc;
+        if ((rc = upload(h, &h->d_tile_pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4, "upload tile piece lists"))) return rc;
+        if ((rc = upload(h, &h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), "upload tile index tables"))) return rc;
+        if ((rc = upload(h, &h->d_tile_fluid, m.tile_fluid.data(), m.tile_fluid.size() * 4, "upload tile fluid ids"))) return rc;
     }
     if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
@@ -238,6 +267,19 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     return UFS_DVM_OK;
 }
 
+// The 35 velocity sums of the current f, which nobody has summed yet (first step, or the caller rewrote f).
+static int enqueue_sums(ufs_dvm_t h, const StepParams& p) {
+    if (h->plan.ring == 4) {
+        CU(launch_tile_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
+        h->parity ^= 1;   // the pass drew its tile tickets from this parity's counter and zeroed the other one
+    } else {
+        CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
+    }
+    h->sums_valid = true;
+    h->launches++;
+    return UFS_DVM_OK;
+}
+
 int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (!h) return UFS_DVM_EINVAL;
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
@@ -245,13 +287,11 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (!(dt > 0) || nsteps < 0) return fail(h, UFS_DVM_EINVAL, "dt must be positive and nsteps >= 0");
     const bool stream = h->plan.ring >= 2 && h->mesh.n_kin > 0;
     for (int s = 0; s < nsteps; s++) {
-        const StepParams p = make_params(h, dt);
         if (stream && !h->sums_valid) {
-            // nobody has summed this f yet (first step, or the caller rewrote it)
-            CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
-            h->sums_valid = true;
-            h->launches++;
+            const int rc = enqueue_sums(h, make_params(h, dt));
+            if (rc) return rc;
         }
+        const StepParams p = make_params(h, dt);
         StepLaunch plan = h->plan;
         plan.ev0 = plan.ev1 = nullptr;
         if (h->prof_on && h->prof_n < ufs_dvm_s::MAX_PROF) {
@@ -274,17 +314,17 @@ int ufs_dvm_moments(ufs_dvm_t h, double* mom_dev) {
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!mom_dev && h->mesh.n_kin > 0) return fail(h, UFS_DVM_EINVAL, "mom_dev is NULL");
-    const StepParams p = make_params(h, 1.0);
     if (h->plan.ring >= 2 && h->mesh.n_kin > 0) {
         if (!h->sums_valid) {
-            CU(launch_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "sums kernel launch");
-            h->sums_valid = true;
-            h->launches++;
+            const int rc = enqueue_sums(h, make_params(h, 1.0));
+            if (rc) return rc;
         }
+        const StepParams p = make_params(h, 1.0);
         CU(launch_moments_from_sums(p, h->d_sums[h->cur], mom_dev, h->stream), "moments kernel launch");
         h->launches++;
         return UFS_DVM_OK;
     }
+    const StepParams p = make_params(h, 1.0);
     CU(launch_moments(h->storage, p, h->f[h->cur], mom_dev, h->stream), "moments kernel launch");
     if (h->mesh.n_kin > 0) h->launches++;
     return UFS_DVM_OK;
@@ -311,6 +351,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
+        cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_tile_fluid);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
     }
     delete h;
@@ -378,6 +419,21 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, doubl
     return ufs_dvm_sync(h);
 }
 
+int ufs_dvm_tiles(ufs_dvm_t h, int64_t* n_tiles, int32_t* pmax, int32_t* hdr, uint32_t* pieces, uint8_t* cellidx,
+                  int32_t* fluid, int64_t* n_fluid_ghosts, int64_t* fluid_leaf) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    if (n_tiles) *n_tiles = (int64_t)m.tiles.size();
+    if (pmax) *pmax = m.tile_pmax;
+    if (hdr) std::memcpy(hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr));
+    if (pieces) std::memcpy(pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4);
+    if (cellidx) std::memcpy(cellidx, m.tile_cellidx.data(), m.tile_cellidx.size());
+    if (fluid && !m.tile_fluid.empty()) std::memcpy(fluid, m.tile_fluid.data(), m.tile_fluid.size() * 4);
+    if (n_fluid_ghosts) *n_fluid_ghosts = (int64_t)m.fluid_leaf.size();
+    if (fluid_leaf) std::memcpy(fluid_leaf, m.fluid_leaf.data(), m.fluid_leaf.size() * 8);
+    return UFS_DVM_OK;
+}
+
 int64_t ufs_dvm_launch_count(ufs_dvm_t h) { return h ? h->launches : 0; }
 
 int ufs_dvm_profile(ufs_dvm_t h, int enable) {
@@ -413,7 +469,8 @@ int ufs_dvm_kernel_info(ufs_dvm_t h, int32_t* threads, int32_t* smem_bytes, int3
 
 const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
     if (!h) return "";
-    return h->plan.ring == 3 ? "k_rows" : h->plan.ring == 2 ? "k_stream" : (h->plan.fast ? "k_step_fast" : "k_step_generic");
+    return h->plan.ring == 4 ? "k_tiles" : h->plan.ring == 3 ? "k_rows" : h->plan.ring == 2 ? "k_stream"
+                             : (h->plan.fast ? "k_step_fast" : "k_step_generic");
 }
 
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }

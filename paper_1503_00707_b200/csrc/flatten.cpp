@@ -384,7 +384,127 @@ int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
         m.n_simple += simple;
     }
     if (!ok) { err = "internal: a kinetic cell has a direction with neither 1 nor 4 sources"; return UFS_DVM_EMESH; }
+
+    // ---- sibling octets among the slabs (tiles): eight consecutive slabs that are the children 0..7 of one parent ----
+    m.octet_start.assign(m.n_kin, 0);
+    for (int64_t s = 0; s + 7 < m.n_kin; s++) {
+        const int64_t j = m.cell_of_slab[s];
+        const uint32_t* c = d.ijk + 3 * j;
+        if (d.level[j] == 0 || ((c[0] | c[1] | c[2]) & 1u)) continue;
+        bool all = true;
+        for (int i = 1; i < 8 && all; i++) {
+            const int64_t q = m.cell_of_slab[s + i];
+            const uint32_t* cq = d.ijk + 3 * q;
+            all = d.level[q] == d.level[j] && cq[0] == c[0] + (i & 1) && cq[1] == c[1] + ((i >> 1) & 1) && cq[2] == c[2] + ((i >> 2) & 1);
+        }
+        m.octet_start[s] = all ? 1 : 0;
+    }
     return UFS_DVM_OK;
+}
+
+namespace {
+
+// Piece list and cell index tables of the tile [s0, s0 + nc) for every octant.  Returns false if an octant needs more
+// than pmax pieces.
+struct TileBuild {
+    uint32_t pieces[8][256];
+    int np[8];
+    uint8_t cidx[8][TILE_CELLS][CELLIDX_BYTES];
+    int32_t fluid[TILE_CELLS][24];
+    bool any_fluid;
+};
+bool make_tile(const FlatMesh& m, int64_t s0, int nc, int pmax, TileBuild& t) {
+    t.any_fluid = false;
+    for (int c = 0; c < TILE_CELLS; c++) for (int k = 0; k < 24; k++) t.fluid[c][k] = -1;
+    for (int o = 0; o < 8; o++) {
+        int np = 0;
+        auto piece = [&](uint32_t code) -> int {
+            for (int i = 0; i < np; i++) if (t.pieces[o][i] == code) return i;
+            if (np < 255) t.pieces[o][np] = code;
+            return np++;
+        };
+        std::memset(t.cidx[o], IDX_NONE, sizeof t.cidx[o]);
+        // own chunks first: piece c is the own chunk of cell c
+        for (int c = 0; c < nc; c++) t.cidx[o][c][0] = (uint8_t)piece((uint32_t)((s0 + c) * 8 + o));
+        for (int c = 0; c < nc; c++) {
+            const CellRec& r = m.recs[s0 + c];
+            uint8_t flags = 0;
+            for (int a = 0; a < 3; a++) {
+                const int dir = 2 * a + (1 - ((o >> a) & 1));  // xi_a > 0: data comes from the low side
+                const int cnt = r.src[dir][1] >= 0 ? 4 : 1;
+                if (cnt == 4) flags |= (uint8_t)(1 << a);
+                for (int k = 0; k < cnt; k++) {
+                    const int32_t code = r.src[dir][k];
+                    const int kind = code >> SRC_SHIFT;
+                    const int64_t idx = code & SRC_INDEX_MASK;
+                    uint8_t e;
+                    if (kind == SRC_FLUID) {
+                        e = IDX_FLUID; flags |= CIDX_FLUID; t.any_fluid = true;
+                        t.fluid[c][dir * 4 + k] = (int32_t)idx;
+                    } else {
+                        uint32_t pc;
+                        if (kind == SRC_SLAB) pc = (uint32_t)(idx * 8 + o);
+                        else if (kind == SRC_MIRROR) pc = (uint32_t)(idx * 8 + (o ^ (1 << a)));  // specular: mirrored octant of the own slab
+                        else pc = PIECE_TABLE | (uint32_t)(idx * 8 + o);
+                        const int pi = piece(pc);
+                        if (pi >= IDX_FLUID) return false;
+                        e = (uint8_t)pi;
+                    }
+                    t.cidx[o][c][4 + 4 * a + k] = e;
+                }
+            }
+            t.cidx[o][c][1] = flags;
+        }
+        if (np > pmax) return false;
+        t.np[o] = np;
+    }
+    return true;
+}
+
+}  // namespace
+
+void build_tiles(FlatMesh& m, int pmax) {
+    m.tile_pmax = pmax;
+    m.tiles.clear(); m.tile_pieces.clear(); m.tile_cellidx.clear(); m.tile_fluid.clear();
+    const bool has_fluid = !m.fluid.empty();
+    // pass 1 (serial, cheap): tile boundaries; pass 2: fill the arrays
+    std::vector<int64_t> start; std::vector<int> count;
+    TileBuild* tb = new TileBuild;
+    for (int64_t s = 0; s < m.n_kin;) {
+        int nc = 0;
+        if (m.octet_start[s] && make_tile(m, s, 8, pmax, *tb)) nc = 8;
+        if (!nc) {
+            // a run of consecutive slabs that stops before the next complete octet and while the piece lists fit
+            nc = 1;
+            while (nc < TILE_CELLS && s + nc < m.n_kin && !m.octet_start[s + nc] && make_tile(m, s, nc + 1, pmax, *tb)) nc++;
+        }
+        start.push_back(s); count.push_back(nc);
+        s += nc;
+    }
+    delete tb;
+    const int64_t nt = (int64_t)start.size();
+    m.tiles.assign(nt, TileHdr{});
+    m.tile_pieces.assign((size_t)nt * 8 * pmax, 0u);
+    m.tile_cellidx.assign((size_t)nt * 8 * TILE_CELLS * CELLIDX_BYTES, IDX_NONE);
+    if (has_fluid) m.tile_fluid.assign((size_t)nt * TILE_CELLS * 24, -1);
+#pragma omp parallel
+    {
+        TileBuild* t = new TileBuild;
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < nt; i++) {
+            make_tile(m, start[i], count[i], pmax, *t);
+            TileHdr& h = m.tiles[i];
+            h.s0 = (int32_t)start[i]; h.nc = count[i];
+            for (int c = 0; c < TILE_CELLS; c++) h.level[c] = c < count[i] ? (uint8_t)m.recs[start[i] + c].level : 0;
+            for (int o = 0; o < 8; o++) {
+                h.np[o] = (uint8_t)t->np[o];
+                std::memcpy(&m.tile_pieces[((size_t)i * 8 + o) * pmax], t->pieces[o], (size_t)t->np[o] * 4);
+                std::memcpy(&m.tile_cellidx[((size_t)i * 8 + o) * TILE_CELLS * CELLIDX_BYTES], t->cidx[o], TILE_CELLS * CELLIDX_BYTES);
+            }
+            if (has_fluid) std::memcpy(&m.tile_fluid[(size_t)i * TILE_CELLS * 24], t->fluid, sizeof t->fluid);
+        }
+        delete t;
+    }
 }
 
 }  // namespace ufs

@@ -66,6 +66,26 @@ struct FluidGhost {          // frozen Maxwellian of a FLUID leaf, separable fac
     double g[3][NV_MAX];     // exp(-(xi_k - u_a)^2 / 2T), canonical index
 };
 
+// ---- tiles (step_tiles.cu): up to TILE_CELLS consecutive slabs stepped together, so that a chunk that is the upwind
+// source of several cells of the tile (siblings of a Morton octet) is brought on chip once.  For each tile
+// and velocity octant (sign group) the flattener lists the distinct source chunks ("pieces") and, per
+// cell, which piece is its own chunk and which pieces are its upwind sources on each axis -- the first-order stencil
+// records of PAPER.md:113-115, deduplicated per tile.
+constexpr int TILE_CELLS = 8;
+constexpr uint32_t PIECE_TABLE = 0x80000000u;  // piece code: bit 31 = inflow ghost table, bits 0..30 = (slab or table) * 8 + octant
+constexpr uint8_t IDX_NONE = 0xFF;             // cell index table: unused source
+constexpr uint8_t IDX_FLUID = 0xFE;            // ... source is a fluid leaf (computed, not copied)
+constexpr int CELLIDX_BYTES = 16;              // per (tile, octant, cell): [0] own piece, [1] flags, [4+4a+k] source k on axis a
+constexpr uint8_t CIDX_FOUR = 0x07;            // flags bits 0..2: axis a has four (finer) sources, each weighted 1/4
+constexpr uint8_t CIDX_FLUID = 0x08;           // flags bit 3: some source of the cell is IDX_FLUID
+struct TileHdr {                               // 32 bytes
+    int32_t s0, nc;                            // first slab, cells
+    uint8_t np[8];                             // pieces per octant
+    uint8_t level[TILE_CELLS];
+    int32_t pad[2];
+};
+static_assert(sizeof(TileHdr) == 32, "TileHdr must be 32 bytes");
+
 struct FlatMesh {
     int64_t n_leaves = 0, n_kin = 0;
     int lmax = 0;
@@ -90,9 +110,20 @@ struct FlatMesh {
     std::vector<double> tables;         // [n_tables][Nv] inflow Maxwellians, SLOT order, fp64
     int64_t n_simple = 0;
     VelLayout vel;
+    // tiles (filled by build_tiles)
+    std::vector<uint8_t> octet_start;       // [n_kin] 1: slabs s..s+7 are the eight leaf children of one parent, all kinetic
+    int tile_pmax = 0;                      // piece-list stride
+    std::vector<TileHdr> tiles;
+    std::vector<uint32_t> tile_pieces;      // [n_tiles][8 octants][tile_pmax]
+    std::vector<uint8_t> tile_cellidx;      // [n_tiles][8 octants][TILE_CELLS][CELLIDX_BYTES]
+    std::vector<int32_t> tile_fluid;        // [n_tiles][TILE_CELLS][24] fluid ghost of source k of direction d (d*4+k), or empty
 };
 
 // Returns UFS_DVM_OK or an error code with a message in `err`.
 int flatten(const ufs_dvm_desc& d, FlatMesh& out, std::string& err);
+
+// Groups the slabs into tiles whose piece lists hold at most `pmax` pieces per octant (complete sibling octets where
+// the mesh has them, else runs of consecutive slabs) and fills the tile arrays of `m`.
+void build_tiles(FlatMesh& m, int pmax);
 
 }  // namespace ufs

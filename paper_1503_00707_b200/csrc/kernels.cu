@@ -569,6 +569,7 @@ int step_plan(int storage, const VelLayout& v, StepLaunch* plan, const char** wh
 
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
     if (p.n_kin == 0) return cudaSuccess;
+    if (plan.ring == 4) return launch_tiles(storage, plan, p, st);
     if (plan.ring == 3) return launch_rows(storage, plan, p, st);
     if (plan.ring == 2) return launch_stream(storage, plan, p, st);
     if (plan.ev0) cudaEventRecord(plan.ev0, st);

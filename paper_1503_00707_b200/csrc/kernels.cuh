@@ -43,15 +43,21 @@ struct StepParams {
     // row kernel (step_rows.cu): |xi_x| of the x ranks and its powers (uniform operands, constant bank)
     double xpow[3][16];         // [r-1][rank] = |xi_x|^r, r = 1..3
     float xf[16];               // |xi_x| in fp32
-    uint32_t smap[12];          // row kernel: its shared-memory map (byte offsets), computed by the launcher
+    uint32_t smap[12];          // row / tile kernel: its shared-memory map (byte offsets), computed by the launcher
+    // tile kernel (step_tiles.cu): the tile records of the flattener
+    const TileHdr* tile_hdr;        // [n_tiles]
+    const uint32_t* tile_pieces;    // [n_tiles][8][tile_pmax]
+    const uint8_t* tile_cellidx;    // [n_tiles][8][TILE_CELLS][CELLIDX_BYTES]
+    const int32_t* tile_fluid;      // [n_tiles][TILE_CELLS][24] or NULL
+    int32_t n_tiles, tile_pmax;
 };
 
 constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used)
 
 struct StepLaunch {
     int32_t threads, smem_bytes, vec, fast;
-    int32_t ring;                  // 3: streaming step, one row per thread (step_rows.cu), 2: streaming step, one
-                                   // vector per thread (step_stream.cu), 0: one CTA per cell (kernels.cu)
+    int32_t ring;                  // 4: tile kernel (step_tiles.cu), 3: streaming step, one row per thread (step_rows.cu),
+                                   // 2: streaming step, one vector per thread (step_stream.cu), 0: one CTA per cell (kernels.cu)
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
     cudaEvent_t ev0, ev1;          // if set: recorded on the stream right before / after the main kernel of the step
 };
@@ -77,6 +83,11 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
 cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 cudaError_t launch_moments_from_sums(const StepParams& p, const double* sums, double* mom, cudaStream_t stream);
+
+// step_tiles.cu: the same step over tiles of up to eight consecutive slabs (shared upwind chunks on chip)
+bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax);
+cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
+cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);

@@ -16,7 +16,6 @@
 // of k_prep) travels in a small ring of cell headers.  The warp that finishes a cell last adds up the per-warp
 // partial sums and writes the cell's 35 velocity sums for the next step.
 #include <cmath>
-#include <cstdlib>
 
 #include "device_util.cuh"
 #include "kernels.cuh"
@@ -463,7 +462,10 @@ __global__ void __launch_bounds__((NG * GW + 1) * 32, 1) k_rows(const StepParams
                     uint32_t ph = ph0 ^ (uint32_t)(wraps & 1);
                     // the producer must have armed the stage's last slot before its barrier's parity means anything
                     const int need = gslot0 + before + (mask ? 4 : 1);
-                    while (slds_i32_volatile(sb + s.issued) < need) __nanosleep(64);
+                    for (uint32_t spins = 0; slds_i32_volatile(sb + s.issued) < need; ) {
+                        __nanosleep(64);
+                        if (++spins > (1u << 24)) __trap();   // seconds without progress: a protocol bug must not hang the GPU
+                    }
                     __threadfence_block();
                     smbar_wait(sb + s.full + 8u * slot, ph);
                     T* const st = reinterpret_cast<T*>(smem_raw + s.ring + (size_t)slot * slot_bytes) + (size_t)r * NHX;
@@ -642,8 +644,6 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan) 
     int ns = 16;
     while (ns >= 4 && rows_smem_bytes(elem, ns, slot, nw, tabn, nr) > ROWS_SMEM_MAX) ns--;
     if (ns < 4) return false;  // a 2:1 face needs four slots in flight at once
-    // UFS_DVM_NS / UFS_DVM_GRID: shallower ring / fewer CTAs, for the sensitivity runs quoted in profiles/
-    if (const char* e = std::getenv("UFS_DVM_NS")) { const int f = std::atoi(e); if (f >= 4 && f < ns) ns = f; }
     *plan = base;
     plan->ring = 3;
     plan->ncw = vi;            // which instantiation
@@ -651,7 +651,6 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan) 
     plan->threads = (nw + 1) * 32;
     plan->smem_bytes = (int32_t)rows_smem_bytes(elem, ns, slot, nw, tabn, nr);
     plan->grid = sm_count;
-    if (const char* e = std::getenv("UFS_DVM_GRID")) { const int f = std::atoi(e); if (f >= 1 && f < sm_count) plan->grid = f; }
     return true;
 }
 
@@ -669,7 +668,3 @@ cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p
 }
 
 }  // namespace ufs
-
-#ifdef UFS_DEBUG_WAIT
-extern "C" int ufs_dvm_debug_read(int* out) { return (int)cudaMemcpyFromSymbol(out, ufs::g_dbg, sizeof(int) * 8); }
-#endif

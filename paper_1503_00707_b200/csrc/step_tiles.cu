@@ -1,0 +1,539 @@
+// step_tiles.cu -- k_tiles: the streaming pass of the DVM step (scheme: step_stream.cu) over TILES of up to eight
+// consecutive slabs.
+//
+// Why tiles.  For one velocity octant (sign group) a cell reads four chunks: its own and the upwind
+// cell's on each axis (first-order stencil records).  For the eight leaf children of one parent
+// (consecutive in N-order) half of those upwind cells are siblings, so a tile that holds the octet needs
+// 20 distinct chunks per octant instead of 32; a coarser neighbour serves four cells with one chunk.  The flattener
+// lists the distinct chunks ("pieces") of every tile and octant (flatten.hpp); here they arrive once by cp.async.bulk
+// and every consumer thread picks its four streams by index.
+//
+// Work decomposition.  A stage is (tile, row block q, octant o): NRP = 48 rows of every piece (a third of a 12x12-row
+// chunk), 8 cells x 48 rows = one velocity row per consumer thread (12 warps).  Pieces live in a ring of NP piece
+// slots allocated in stage order (a stage takes np <= pmax consecutive slots, modulo NP); stage k uses barrier pair
+// k mod NSTG.  Four producer warps issue the copies of every stage together (piece i by lane i/4 of warp i%4), one of
+// them also draws the tile tickets and publishes the tile header (cells, levels, Maxwellian factor tables of k_prep).
+// A thread finishes its row exactly like k_rows:  f' = B f + Cx_k (fX - f) + Cy fY + Cz fZ + W gx_k  (Eq. 2,
+// PAPER.md:103, with the BGK relaxation of PAPER.md:231 folded in), one store, four fp64 x sums of the row.  Over the
+// eight octants of a row block the row sums are kept as 16 sign-weighted combinations (no octant-indexed registers);
+// after the block they are expanded with the row's |xi_y|, |xi_z| to the cell's 35 velocity sums (stream_common.cuh),
+// reduced over 16 lanes by a halving butterfly and added into shared memory; the last block writes them out.
+#include <cmath>
+
+#include "device_util.cuh"
+#include "kernels.cuh"
+#include "stream_common.cuh"
+
+namespace ufs {
+namespace {
+
+constexpr int NRP = 48;                 // rows of a piece
+constexpr int THX = 12;                 // values of a row (nh_x)
+constexpr int N_PROD = 4;               // producer warps: warps 0..3
+constexpr int N_CONS = 12;              // consumer warps: warps 4..15
+constexpr int NSTG = 8;                 // stage barrier pairs / stage descriptors
+constexpr int TSLOTS = 3;               // tile header slots
+constexpr int DESC_BYTES = TILE_CELLS * CELLIDX_BYTES + 16;   // cell index tables, then the stage's first piece slot
+constexpr int THDR_NEXT = 36;           // tile header: TileHdr (32 B), tile id (or -1: stop), next tile id,
+constexpr int THDR_FLUID = 64;          //   fluid ghost ids int32[8][24],
+constexpr int THDR_TAB = 896;           //   factor tables [8][tabn] of the storage type
+constexpr int RED_DOUBLES = TILE_CELLS * 3 * SUMS_STRIDE;     // partial sums: [cell][16-lane group][36]
+
+struct TilesSmem { uint32_t ring, desc, thdr, red, full, empty, tinfo, ttab, tempty, total, thdr_bytes; };
+__host__ __device__ inline TilesSmem tiles_map(size_t elem, int np, int tabn) {
+    TilesSmem s;
+    size_t off = 0;
+    s.ring = 0; off += (size_t)np * NRP * THX * elem;
+    s.desc = (uint32_t)off; off += (size_t)NSTG * DESC_BYTES;
+    off = (off + 127) & ~(size_t)127;
+    s.thdr_bytes = (uint32_t)((THDR_TAB + (size_t)TILE_CELLS * tabn * elem + 127) & ~(size_t)127);
+    s.thdr = (uint32_t)off; off += (size_t)TSLOTS * s.thdr_bytes;
+    s.red = (uint32_t)off; off += (size_t)2 * RED_DOUBLES * 8;
+    s.full = (uint32_t)off; off += NSTG * 8;
+    s.empty = (uint32_t)off; off += NSTG * 8;
+    s.tinfo = (uint32_t)off; off += TSLOTS * 8;
+    s.ttab = (uint32_t)off; off += TSLOTS * 8;
+    s.tempty = (uint32_t)off; off += TSLOTS * 8;
+    s.total = (uint32_t)((off + 127) & ~(size_t)127);
+    return s;
+}
+
+template <typename T> __device__ __forceinline__ T tx_of(const StepParams& p, int k);
+template <> __device__ __forceinline__ float tx_of<float>(const StepParams& p, int k) { return p.xf[k]; }
+template <> __device__ __forceinline__ double tx_of<double>(const StepParams& p, int k) { return p.xpow[0][k]; }
+
+// halving butterfly over the 16 lanes of a group: 36 -> 18 -> 9 -> 5 -> 3 values per lane (stream_common.cuh: halve)
+__device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
+    halve<36, 8>(v, lane);
+    halve<18, 4>(v, lane);
+    halve<9, 2>(v, lane);
+    halve<5, 1>(v, lane);
+}
+
+// Upwind values of a kinetic/fluid face (reading G13): pointwise Maxwellian of the fluid leaf's frozen
+// moments from its separable factors; j = 16-byte vector of the row, (ry, rz) = ranks of |xi_y|, |xi_z|.
+template <typename T>
+__device__ __forceinline__ void fluid_row_vec(const StepParams& p, int ghost, int o, int j, int ry, int rz, T (&v)[V16<T>::N]) {
+    constexpr int VEC = V16<T>::N;
+    const FluidGhost* g = p.fluid + ghost;
+    const int kz = ((o >> 2) & 1) ? p.nh[2] + rz : p.nh[2] - 1 - rz;
+    const int ky = ((o >> 1) & 1) ? p.nh[1] + ry : p.nh[1] - 1 - ry;
+    const double b = g->amp * g->g[2][kz] * g->g[1][ky];
+#pragma unroll
+    for (int i = 0; i < VEC; i++) {
+        const int kx = (o & 1) ? p.nh[0] + j * VEC + i : p.nh[0] - 1 - j * VEC - i;
+        v[i] = (T)(b * g->g[0][kx]);
+    }
+}
+
+template <typename T, bool FLUID, bool SUMS_ONLY>
+__global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepParams p) {
+    constexpr int VEC = V16<T>::N, RV = THX / VEC;
+    constexpr uint32_t ROWB = THX * sizeof(T);          // bytes of a row
+    constexpr uint32_t PB = NRP * ROWB;                 // bytes of a piece
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const uint32_t sb = smem_u32(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int NP = p.ring_stages;                       // piece slots of the ring
+    const int nhp = nhp_of(p.nh), tabn = tabn_of(p.nh);
+    const int NR = p.nh[1] * p.nh[2];                   // rows of an octant chunk
+    const int NQ = NR / NRP;                            // row blocks
+    const int CH = NR * THX;                            // elements of an octant chunk
+    // shared-memory map (kernel parameters: constant bank, no registers)
+    const uint32_t o_desc = p.smap[1], o_thdr = p.smap[2], o_red = p.smap[3], o_full = p.smap[4], o_empty = p.smap[5],
+                   o_tinfo = p.smap[6], o_ttab = p.smap[7], o_tempty = p.smap[8], thdr_bytes = p.smap[10];
+
+    if (tid == 0) {
+        for (int i = 0; i < NSTG; i++) {
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + o_full) + i, N_PROD);
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + o_empty) + i, N_CONS);
+        }
+        for (int i = 0; i < TSLOTS; i++) {
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + o_tinfo) + i, 1);
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + o_ttab) + i, 1);
+            mbar_init(reinterpret_cast<uint64_t*>(smem_raw + o_tempty) + i, N_CONS + N_PROD - 1);
+        }
+        mbar_init_fence();
+        if (blockIdx.x == 0) *p.counter_reset = 0;  // the other launch parity's ticket counter
+    }
+    __syncthreads();
+
+    if (warp < N_PROD) {
+        // =========================================================== producer warps
+        const int w = warp;
+        const T* fin = reinterpret_cast<const T*>(p.f_in);
+        const int my_piece = 4 * lane + w;          // the piece of every stage this lane copies
+        uint32_t code[8], code_nx[8];               // its source chunk per octant: current / next tile
+        int hw_nx = 0;                              // (warp 0, lanes 0..7) word `lane` of the next tile's TileHdr
+        int tk_cur = 0, tk_nx_raw = 0;              // (warp 0) ticket of the current tile; lane 0: the next tile's (atomic in flight)
+        // ring bookkeeping, identical in the four warps: pieces allocated / released so far, next stage to be released
+        uint32_t alloc = 0, rel = 0;
+        int head = 0;
+        int k = 0, r = 0, rq = 0;                   // stage counters: next to issue, next to release, r within its tile
+        bool r_prev = false;                        // stage r belongs to the previous tile
+        unsigned long long np_cur = 0, np_prev = 0; // pieces per octant (8 bytes) of the current / previous tile
+        auto load_codes = [&](int tile, uint32_t (&c)[8]) {
+#pragma unroll
+            for (int o = 0; o < 8; o++)
+                c[o] = (!SUMS_ONLY && tile < p.n_tiles && my_piece < p.tile_pmax)
+                           ? __ldg(p.tile_pieces + ((size_t)tile * 8 + o) * p.tile_pmax + my_piece) : 0u;
+        };
+        if (w == 0) {
+            int t0 = 0, t1 = 0;
+            if (lane == 0) { t0 = atomicAdd(p.counter, 1); t1 = atomicAdd(p.counter, 1); }
+            tk_cur = __shfl_sync(0xffffffffu, t0, 0);
+            tk_nx_raw = t1;
+            hw_nx = (lane < 8 && tk_cur < p.n_tiles) ? __ldg(reinterpret_cast<const int*>(p.tile_hdr + tk_cur) + lane) : 0;
+        }
+        for (int n = 0;; n++) {
+            const int ts = n % TSLOTS;
+            const uint32_t tph = (uint32_t)((n / TSLOTS) & 1);
+            const uint32_t hdr = sb + o_thdr + ts * thdr_bytes;
+            int tile, next, s0, nc;
+            if (w == 0) {
+                // publish the header of tile n: its TileHdr came in a tile ago, the ticket of tile n + 1 as well
+                smbar_wait(sb + o_tempty + 8u * ts, tph ^ 1u);
+                tile = tk_cur < p.n_tiles ? tk_cur : -1;
+                next = __shfl_sync(0xffffffffu, tk_nx_raw, 0);   // drawn a tile ago
+                const int hw = hw_nx;
+                if (lane < 8) ssts_i32(hdr + 4u * lane, hw);
+                if (lane == 8) ssts_i32(hdr + 32u, tile);
+                if (lane == 9) ssts_i32(hdr + THDR_NEXT, next);
+                s0 = __shfl_sync(0xffffffffu, hw, 0);
+                nc = __shfl_sync(0xffffffffu, hw, 1);
+                np_prev = np_cur;
+                np_cur = (unsigned long long)(uint32_t)__shfl_sync(0xffffffffu, hw, 2)
+                         | ((unsigned long long)(uint32_t)__shfl_sync(0xffffffffu, hw, 3) << 32);
+                __syncwarp();
+                if (lane == 0) {
+                    smbar_arrive(sb + o_tinfo + 8u * ts);
+                    const uint32_t tb = sb + o_ttab + 8u * ts;
+                    const uint32_t tab_bytes = (p.collide && !SUMS_ONLY && tile >= 0) ? (uint32_t)(nc * tabn) * (uint32_t)sizeof(T) : 0u;
+                    const uint32_t fl_bytes = (FLUID && tile >= 0) ? (uint32_t)(TILE_CELLS * 24 * 4) : 0u;
+                    if (tab_bytes + fl_bytes) {
+                        smbar_arrive_expect_tx(tb, tab_bytes + fl_bytes);
+                        if (tab_bytes) sbulk_g2s(hdr + THDR_TAB, reinterpret_cast<const T*>(p.tabs) + (size_t)s0 * tabn, tab_bytes, tb);
+                        if (fl_bytes) sbulk_g2s(hdr + THDR_FLUID, p.tile_fluid + (size_t)tile * TILE_CELLS * 24, fl_bytes, tb);
+                    } else {
+                        smbar_arrive(tb);
+                    }
+                }
+                if (tile < 0) break;
+                // the ticket after the next (its result is read a tile from now) and the next tile's header words
+                tk_cur = next;
+                if (lane == 0) tk_nx_raw = atomicAdd(p.counter, 1);
+                hw_nx = (lane < 8 && next < p.n_tiles) ? __ldg(reinterpret_cast<const int*>(p.tile_hdr + next) + lane) : 0;
+            } else {
+                smbar_wait(sb + o_tinfo + 8u * ts, tph);
+                s0 = slds_i32(hdr + 0u);
+                nc = slds_i32(hdr + 4u);
+                np_prev = np_cur;
+                np_cur = (unsigned long long)(uint32_t)slds_i32(hdr + 8u) | ((unsigned long long)(uint32_t)slds_i32(hdr + 12u) << 32);
+                tile = slds_i32(hdr + 32u);
+                next = slds_i32(hdr + THDR_NEXT);
+                __syncwarp();
+                if (lane == 0) smbar_arrive(sb + o_tempty + 8u * ts);   // everything needed is in registers
+                if (tile < 0) break;
+            }
+            if (SUMS_ONLY) np_cur = (unsigned long long)nc * 0x0101010101010101ull;   // own chunks only
+            if (n == 0) load_codes(tile, code);
+            else {
+#pragma unroll
+                for (int o = 0; o < 8; o++) code[o] = code_nx[o];
+            }
+            load_codes(next, code_nx);   // in flight during this tile's stages
+            r_prev = (r < k);            // stages not yet released belong to the tile that just ended (8 NQ >= NSTG)
+            for (int q = 0; q < NQ; q++) {
+#pragma unroll
+                for (int o = 0; o < 8; o++) {
+                    const int npk = (int)((np_cur >> (8 * o)) & 0xffull);
+                    // ring space: piece slots and the barrier pair of stage k
+                    while (k - r >= NSTG || alloc + (uint32_t)npk - rel > (uint32_t)NP) {
+                        smbar_wait(sb + o_empty + 8u * (r % NSTG), (uint32_t)((r / NSTG) & 1));
+                        rel += (uint32_t)(((r_prev ? np_prev : np_cur) >> (8 * (rq & 7))) & 0xffull);
+                        r++;
+                        if (++rq == 8 * NQ) { rq = 0; r_prev = false; }
+                    }
+                    const int slot = k % NSTG;
+                    const uint32_t fb = sb + o_full + 8u * slot;
+                    const uint32_t dsc = sb + o_desc + slot * DESC_BYTES;
+                    const int mine = npk > w ? (npk + 3 - w) >> 2 : 0;   // pieces this warp copies
+                    if (lane == 0) {
+                        if (w == 0) ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
+                        const uint32_t extra = (w == 0 && !SUMS_ONLY) ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u;
+                        smbar_arrive_expect_tx(fb, (uint32_t)mine * PB + extra);
+                        if (extra) sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), extra, fb);
+                    }
+                    __syncwarp();
+                    if (my_piece < npk) {
+                        const uint32_t c = SUMS_ONLY ? (uint32_t)((s0 + my_piece) * 8 + o) : code[o];
+                        const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
+                                       + (size_t)(c & ~PIECE_TABLE) * (size_t)CH + (size_t)q * (NRP * THX);
+                        int ps = head + my_piece;
+                        if (ps >= NP) ps -= NP;
+                        sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
+                    }
+                    head += npk;
+                    if (head >= NP) head -= NP;
+                    alloc += (uint32_t)npk;
+                    k++;
+                }
+            }
+        }
+        return;
+    }
+
+    // =============================================================== consumer warps: thread = (cell c, row r of the piece)
+    const int ct = tid - N_PROD * 32;
+    const int c = ct / NRP, rr = ct % NRP;
+    const int gi = rr >> 4;                          // 16-lane group of the cell
+    const int ry = rr % p.nh[1], rzl = rr / p.nh[1]; // rank of |xi_y|; rank of |xi_z| inside the row block
+    const double ay = p.vel->xi[1][p.nh[1] + ry];
+    const uint32_t rowoff = (uint32_t)rr * ROWB;
+    const int triple = (warp - N_PROD) / 3;          // three warps share two cells: named barrier 1 + triple
+    int k = 0;
+    for (int n = 0;; n++) {
+        const int ts = n % TSLOTS;
+        const uint32_t hdr = o_thdr + ts * thdr_bytes;   // offset from smem_raw
+        smbar_wait(sb + o_ttab + 8u * ts, (uint32_t)((n / TSLOTS) & 1));
+        const int tile = *reinterpret_cast<const int*>(smem_raw + hdr + 32);
+        if (tile < 0) break;
+        const int s0 = *reinterpret_cast<const int*>(smem_raw + hdr);
+        const int nc = *reinterpret_cast<const int*>(smem_raw + hdr + 4);
+        const bool active = c < nc;
+        const int level = smem_raw[hdr + 16 + c];
+        const T* tab = reinterpret_cast<const T*>(smem_raw + hdr + THDR_TAB) + c * tabn;
+        const double dth = p.dt * p.inv_len * (double)(1 << level);   // dt / h
+        const T omega = (p.collide && !SUMS_ONLY && active) ? tab[6 * nhp] : T(0);
+        const double om1 = 1.0 - (double)omega, omd = om1 * dth;
+        const T sxc = (T)omd;                         // times |xi_x,k| : the x coefficient
+        const T cy = (T)(omd * ay);
+        T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)(s0 + c) * p.Nv;
+        double* const red = reinterpret_cast<double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)(c * 3 + gi) * SUMS_STRIDE;
+        for (int q = 0; q < NQ; q++) {
+            const int rz = q * (NRP / p.nh[1]) + rzl;
+            const double az = p.vel->xi[2][p.nh[2] + rz];
+            const T cz = (T)(omd * az);
+            const T base = (T)(om1 - omd * (ay + az));
+            const int row = q * NRP + rr;             // row of the octant chunk
+            // the 16 sign-weighted combinations of the row sums s_k = sum_x |xi_x|^k f' over the eight octants
+            double E0 = 0, Ey = 0, Ez = 0, Eyz = 0, F0 = 0, Fx = 0, Fy = 0, Fxy = 0, Fz = 0, Fxz = 0, G0 = 0, Gx = 0, Gy = 0, Gz = 0, K0 = 0, Kx = 0;
+#pragma unroll 1
+            for (int o = 0; o < 8; o++) {
+                const int slot = k % NSTG;
+                smbar_wait(sb + o_full + 8u * slot, (uint32_t)((k / NSTG) & 1));
+                double s0_ = 0, s1_ = 0, s2_ = 0, s3_ = 0;
+                if (active) {
+                    const unsigned char* dsc = smem_raw + o_desc + slot * DESC_BYTES;
+                    const int head = *reinterpret_cast<const int*>(dsc + TILE_CELLS * CELLIDX_BYTES);
+                    uint4 ix;
+                    if (SUMS_ONLY) ix = make_uint4((uint32_t)c, 0u, 0u, 0u);
+                    else ix = *reinterpret_cast<const uint4*>(dsc + c * CELLIDX_BYTES);
+                    auto addr_of = [&](uint32_t b) -> const T* {
+                        int ps = head + (int)b;
+                        if (ps >= NP) ps -= NP;
+                        return reinterpret_cast<const T*>(smem_raw + (uint32_t)ps * PB + rowoff);
+                    };
+                    const T* a_own = addr_of(ix.x & 0xffu);
+                    const uint32_t flags = (ix.x >> 8) & 0xffu;
+                    T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX;
+                    T wb = T(0);
+                    const T* gxrow = tab + (o & 1) * nhp;
+                    if (p.collide && !SUMS_ONLY) wb = omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rz] * tab[(2 + ((o >> 1) & 1)) * nhp + ry]);
+                    if (SUMS_ONLY) {
+#pragma unroll
+                        for (int j = 0; j < RV; j++) {
+                            T own[VEC];
+                            lds16(a_own + j * VEC, own);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const int kk = j * VEC + i;
+                                const double d = (double)own[i];
+                                s0_ += d;
+                                s1_ = fma(p.xpow[0][kk], d, s1_);
+                                s2_ = fma(p.xpow[1][kk], d, s2_);
+                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                            }
+                        }
+                    } else if (flags == 0) {
+                        // every upwind source is one piece
+                        const T* a_x = addr_of(ix.y & 0xffu);
+                        const T* a_y = addr_of(ix.z & 0xffu);
+                        const T* a_z = addr_of(ix.w & 0xffu);
+#pragma unroll
+                        for (int j = 0; j < RV; j++) {
+                            T own[VEC], X[VEC], Y[VEC], Z[VEC], out[VEC];
+                            lds16(a_own + j * VEC, own);
+                            lds16(a_x + j * VEC, X);
+                            lds16(a_y + j * VEC, Y);
+                            lds16(a_z + j * VEC, Z);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                out[i] = base * own[i] + cx * (X[i] - own[i]) + cy * Y[i] + cz * Z[i];
+                            }
+                            if (p.collide) {
+                                T gx[VEC];
+                                lds16(gxrow + j * VEC, gx);
+#pragma unroll
+                                for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+                            }
+                            stg16_cs(gdst + j * VEC, out);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const int kk = j * VEC + i;
+                                const double d = (double)out[i];
+                                s0_ += d;
+                                s1_ = fma(p.xpow[0][kk], d, s1_);
+                                s2_ = fma(p.xpow[1][kk], d, s2_);
+                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                            }
+                        }
+                    } else {
+                        // 2:1 faces towards finer leaves (four sources, each weighted 1/4: reading G3) and / or fluid leaves
+                        const uint32_t words[3] = {ix.y, ix.z, ix.w};
+                        const int* fl = reinterpret_cast<const int*>(smem_raw + hdr + THDR_FLUID) + c * 24;
+#pragma unroll 1
+                        for (int j = 0; j < RV; j++) {
+                            T own[VEC], S[3][VEC], out[VEC];
+                            lds16(a_own + j * VEC, own);
+#pragma unroll
+                            for (int a = 0; a < 3; a++) {
+                                const int nsrc = (flags >> a) & 1u ? 4 : 1;
+                                const int dir = 2 * a + (1 - ((o >> a) & 1));
+#pragma unroll
+                                for (int i = 0; i < VEC; i++) S[a][i] = T(0);
+                                for (int m = 0; m < nsrc; m++) {
+                                    const uint32_t b = (words[a] >> (8 * m)) & 0xffu;
+                                    T v[VEC];
+                                    if (FLUID && b == IDX_FLUID) fluid_row_vec<T>(p, fl[dir * 4 + m], o, j, ry, rz, v);
+                                    else lds16(addr_of(b) + j * VEC, v);
+#pragma unroll
+                                    for (int i = 0; i < VEC; i++) S[a][i] += v[i];
+                                }
+                                if (nsrc == 4) {
+#pragma unroll
+                                    for (int i = 0; i < VEC; i++) S[a][i] *= T(0.25);
+                                }
+                            }
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                out[i] = base * own[i] + cx * (S[0][i] - own[i]) + cy * S[1][i] + cz * S[2][i];
+                            }
+                            if (p.collide) {
+                                T gx[VEC];
+                                lds16(gxrow + j * VEC, gx);
+#pragma unroll
+                                for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+                            }
+                            stg16_cs(gdst + j * VEC, out);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const int kk = j * VEC + i;
+                                const double d = (double)out[i];
+                                s0_ += d;
+                                s1_ = fma(p.xpow[0][kk], d, s1_);
+                                s2_ = fma(p.xpow[1][kk], d, s2_);
+                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) smbar_arrive(sb + o_empty + 8u * slot);
+                k++;
+                // signs of the octant as doubles; fold the row sums into the 16 combinations
+                const double sx = (o & 1) ? 1.0 : -1.0, sy = (o & 2) ? 1.0 : -1.0, sz = (o & 4) ? 1.0 : -1.0;
+                const double sxy = sx * sy, sxz = sx * sz, syz = sy * sz;
+                E0 += s0_; Ey = fma(sy, s0_, Ey); Ez = fma(sz, s0_, Ez); Eyz = fma(syz, s0_, Eyz);
+                F0 += s1_; Fx = fma(sx, s1_, Fx); Fy = fma(sy, s1_, Fy); Fxy = fma(sxy, s1_, Fxy); Fz = fma(sz, s1_, Fz); Fxz = fma(sxz, s1_, Fxz);
+                G0 += s2_; Gx = fma(sx, s2_, Gx); Gy = fma(sy, s2_, Gy); Gz = fma(sz, s2_, Gz);
+                K0 += s3_; Kx = fma(sx, s3_, Kx);
+            }
+            // expand to the 35 sums of this row block (layout: stream_common.cuh) ...
+            double v[36];
+            const double r2 = fma(ay, ay, az * az);
+            v[0] = E0; v[1] = Fx; v[2] = ay * Ey; v[3] = az * Ez; v[4] = fma(r2, E0, G0);
+#pragma unroll
+            for (int s = 0; s < 2; s++) {
+                const double sp = s ? 1.0 : -1.0;     // sum over the octants with sign s on the axis: (all + sp * signed) / 2
+                const double f0 = 0.5 * fma(sp, Fx, F0);
+                v[g_index(0, s, 0)] = f0;
+                v[g_index(0, s, 1)] = 0.5 * fma(sp, G0, Gx);
+                v[g_index(0, s, 2)] = 0.5 * ay * fma(sp, Fxy, Fy);
+                v[g_index(0, s, 3)] = 0.5 * az * fma(sp, Fxz, Fz);
+                v[g_index(0, s, 4)] = fma(r2, f0, 0.5 * fma(sp, Kx, K0));
+                const double ey = 0.5 * ay * fma(sp, Ey, E0);
+                v[g_index(1, s, 0)] = ey;
+                v[g_index(1, s, 1)] = 0.5 * ay * fma(sp, Fxy, Fx);
+                v[g_index(1, s, 2)] = 0.5 * ay * ay * fma(sp, E0, Ey);
+                v[g_index(1, s, 3)] = 0.5 * ay * az * fma(sp, Eyz, Ez);
+                v[g_index(1, s, 4)] = fma(r2, ey, 0.5 * ay * fma(sp, Gy, G0));
+                const double ez = 0.5 * az * fma(sp, Ez, E0);
+                v[g_index(2, s, 0)] = ez;
+                v[g_index(2, s, 1)] = 0.5 * az * fma(sp, Fxz, Fx);
+                v[g_index(2, s, 2)] = 0.5 * az * ay * fma(sp, Eyz, Ey);
+                v[g_index(2, s, 3)] = 0.5 * az * az * fma(sp, E0, Ez);
+                v[g_index(2, s, 4)] = fma(r2, ez, 0.5 * az * fma(sp, Gz, G0));
+            }
+            v[35] = 0.0;
+            // ... reduce over the 16 lanes of the group and add into the group's partial sums (one owner lane per entry)
+            group16_reduce(v, lane);
+            {
+                const int b0 = lane & 1, b1 = (lane >> 1) & 1, b2 = (lane >> 2) & 1, b3 = (lane >> 3) & 1;
+#pragma unroll
+                for (int t = 0; t < 3; t++) {
+                    const int l4 = t + 3 * b0;
+                    if (l4 < (b1 ? 4 : 5)) {
+                        const int j = l4 + 5 * b1 + 9 * b2 + 18 * b3;
+                        if (q == 0) red[j] = v[t];
+                        else red[j] += v[t];
+                    }
+                }
+            }
+        }
+        // the three warps that share two cells meet; then the cells' sums go out
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + triple), "r"(96) : "memory");
+        {
+            const int u = ct - 96 * triple;
+            if (u < 2 * SUMS_STRIDE) {
+                const int cc = 2 * triple + u / SUMS_STRIDE, j = u % SUMS_STRIDE;
+                if (cc < nc) {
+                    const double* rp = reinterpret_cast<const double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)cc * 3 * SUMS_STRIDE + j;
+                    p.sums_out[(int64_t)(s0 + cc) * SUMS_STRIDE + j] = rp[0] + rp[SUMS_STRIDE] + rp[2 * SUMS_STRIDE];
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) smbar_arrive(sb + o_tempty + 8u * ts);
+    }
+}
+
+constexpr size_t TILES_SMEM_MAX = 227 * 1024;
+
+template <typename T, bool FLUID, bool SUMS_ONLY>
+cudaError_t launch_tiles_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st, bool timed) {
+    auto kfn = k_tiles<T, FLUID, SUMS_ONLY>;
+    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    const int grid = p.n_tiles < plan.grid ? p.n_tiles : plan.grid;
+    StepParams q = p;
+    const TilesSmem m = tiles_map(sizeof(T), plan.stages, tabn_of(p.nh));
+    const uint32_t v[11] = {m.ring, m.desc, m.thdr, m.red, m.full, m.empty, m.tinfo, m.ttab, m.tempty, m.total, m.thdr_bytes};
+    for (int i = 0; i < 11; i++) q.smap[i] = v[i];
+    q.ring_stages = plan.stages;
+    if (timed && plan.ev0) cudaEventRecord(plan.ev0, st);
+    kfn<<<grid, (N_PROD + N_CONS) * 32, plan.smem_bytes, st>>>(q);
+    if (timed && plan.ev1) cudaEventRecord(plan.ev1, st);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// Launch geometry of the tile kernel, or false if the velocity grid does not fit it (12 x-ranks per row, whole row
+// blocks of 48 rows, octant layout); *pmax = pieces a tile may list per octant (two stages must fit the ring).
+bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax) {
+    if (!v.fast || v.nh[0] != THX) return false;
+    const int nr = v.nh[1] * v.nh[2];
+    if (nr % NRP != 0 || NRP % v.nh[1] != 0 || (nr / NRP) * 8 < NSTG) return false;
+    for (int a = 0; a < 3; a++)
+        if (v.nv[a] > 32) return false;
+    StepLaunch base{};
+    if (!stream_plan(storage, v, sm_count, &base)) return false;   // k_prep / fallbacks share its checks
+    const size_t elem = storage == UFS_STORE_F32 ? 4 : 8;
+    const int32_t nh[3] = {v.nh[0], v.nh[1], v.nh[2]};
+    const int tabn = tabn_of(nh);
+    int np = 255;
+    while (np >= 26 && tiles_map(elem, np, tabn).total > TILES_SMEM_MAX) np--;
+    if (np < 26) return false;           // a single cell may need 13 pieces per octant; two stages must fit
+    *plan = base;
+    plan->ring = 4;
+    plan->stages = np;                   // piece slots of the ring
+    plan->threads = (N_PROD + N_CONS) * 32;
+    plan->smem_bytes = (int32_t)tiles_map(elem, np, tabn).total;
+    plan->grid = sm_count;
+    *pmax = np / 2 < 40 ? np / 2 : 40;
+    return true;
+}
+
+cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t st) {
+    if (p.n_kin == 0) return cudaSuccess;
+    cudaError_t e = launch_prep(storage, p, st);
+    if (e != cudaSuccess) return e;
+    if (storage == UFS_STORE_F32)
+        return p.tile_fluid ? launch_tiles_t<float, true, false>(plan, p, st, true) : launch_tiles_t<float, false, false>(plan, p, st, true);
+    return p.tile_fluid ? launch_tiles_t<double, true, false>(plan, p, st, true) : launch_tiles_t<double, false, false>(plan, p, st, true);
+}
+
+// sums[n_kin][SUMS_STRIDE] of an f the caller has just written: the same kernel, own chunks only, no store
+cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t st) {
+    if (p.n_kin == 0) return cudaSuccess;
+    StepParams q = p;
+    q.f_in = f;
+    q.sums_out = sums;
+    if (storage == UFS_STORE_F32) return launch_tiles_t<float, false, true>(plan, q, st, false);
+    return launch_tiles_t<double, false, true>(plan, q, st, false);
+}
+
+}  // namespace ufs

@@ -25,7 +25,7 @@ pytestmark = pytest.mark.gpu
 TOL_F32 = 2e-5     # north star: relative L-infinity, fp32 storage with fp64 moment accumulation
 TOL_F64 = 1e-12    # north star: fp64 storage
 S_WIN = 3          # steps = rings of the window
-STEP_KERNEL = "k_rows"   # the streaming kernel every 24^3 configuration must get (no silent fallback)
+STEP_KERNEL = "k_tiles"   # the streaming kernel every 24^3 configuration must get (no silent fallback)
 
 
 def _need_device_memory(case):

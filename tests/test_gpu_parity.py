@@ -117,6 +117,24 @@ def test_kernel_selection_and_parity_on_other_even_grids(nv, storage, kernel):
     check(case, 3, TOL[storage], storage=storage, f0=f0)
 
 
+@pytest.mark.parametrize("cfg,kernel", [(3, "rows"), (4, "rows"), (5, "rows"), (4, "stream"), (3, "cell")])
+def test_fallback_kernels_on_the_24_cubed_grid(cfg, kernel, monkeypatch):
+    """24^3 grids get k_tiles; UFS_DVM_KERNEL forces the kernels that serve the other grids: they must stay right."""
+    monkeypatch.setenv("UFS_DVM_KERNEL", kernel)
+    case = inputs.small(cfg)
+    st = B.DvmStepper(case)
+    assert B.ufs_dvm_kernel_name(st.h) == {"rows": "k_rows", "stream": "k_stream", "cell": "k_step_fast"}[kernel]
+    st.close()
+    check(case, case.nsteps, TOL[case.storage])
+
+
+def test_small_configs_use_the_tile_kernel():
+    for cfg in (2, 3, 4, 5):
+        st = B.DvmStepper(inputs.small(cfg))
+        assert B.ufs_dvm_kernel_name(st.h) == "k_tiles"
+        st.close()
+
+
 def test_specular_box_with_odd_grid_generic_path():
     lv, ijk = inputs.build_tree(2, 2, {}, P)
     case = periodic_case(lv, ijk, nv=(5, 5, 5), bc=(inputs.BC_SPECULAR,) * 6, kn=0.3)
