@@ -506,6 +506,72 @@ void oracle_dvm_boundary_counts(const oracle_t *o, int64_t counts[5]) {
     }
 }
 
+/* ---- mesh change: f of a new leaf set from f of the old one ("steps 2 and 4 are
+ * redone each time the spatial mesh is changed").  The paper does not say how f is carried over; reading G20
+ * (DESIGN.md), the one consistent with the first-order piecewise-constant scheme (G2): the new value is the VOLUME
+ * AVERAGE over the new leaf of the old piecewise-constant field --
+ *   an unchanged leaf keeps its f; a leaf created by refinement takes the value of the old leaf that covers it
+ *   (injection); a leaf created by coarsening takes sum_k (V_k / V_new) f_k over the old leaves k inside it;
+ *   where the old covering leaf was FLUID the field is the Maxwellian of its frozen moments (G13).
+ * One new leaf and one velocity at a time, plain recursion over the octree. */
+static int remap_add(const oracle_t *old, const double *f_old, int level, int64_t cx, int64_t cy, int64_t cz, double wgt, double *acc) {
+    const int64_t q = find_leaf(old, level, cx, cy, cz);
+    if (q >= 0) {
+        if (old->kind[q] == ORA_SOLID) return ORA_EINVAL;
+        const int nx = old->d.nv[0], ny = old->d.nv[1], nz = old->d.nv[2];
+        for (int kz = 0; kz < nz; kz++) for (int ky = 0; ky < ny; ky++) for (int kx = 0; kx < nx; kx++) {
+            const int64_t i = ((int64_t)kz * ny + ky) * nx + kx;
+            const double v = old->kind[q] == ORA_KINETIC ? f_old[old->row_of_leaf[q] * old->Nv + i]
+                                                         : maxwell_point(old->fluid + 5 * q, old->xi[0][kx], old->xi[1][ky], old->xi[2][kz]);
+            acc[i] += wgt * v;
+        }
+        return ORA_OK;
+    }
+    if (level >= 18) return ORA_EMESH; /* nothing of the old mesh lies here */
+    for (int d = 0; d < 8; d++) {
+        int rc = remap_add(old, f_old, level + 1, 2 * cx + (d & 1), 2 * cy + ((d >> 1) & 1), 2 * cz + ((d >> 2) & 1), wgt / 8.0, acc);
+        if (rc) return rc;
+    }
+    return ORA_OK;
+}
+
+/* f_old: [old n_kinetic][Nv], f_new: [new n_kinetic][Nv]; both meshes must carry the same velocity grid */
+int oracle_dvm_remap(const oracle_t *old, const oracle_t *neu, const double *f_old, double *f_new) {
+    for (int a = 0; a < 3; a++)
+        if (old->d.nv[a] != neu->d.nv[a] || old->d.vmin[a] != neu->d.vmin[a] || old->d.vmax[a] != neu->d.vmax[a]) return ORA_EINVAL;
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t r = 0; r < neu->n_kin; r++) {
+        const int64_t j = neu->kin_leaf[r];
+        const int l = neu->level[j];
+        const int64_t c[3] = {neu->ijk[3 * j], neu->ijk[3 * j + 1], neu->ijk[3 * j + 2]};
+        double *out = f_new + r * neu->Nv;
+        for (int64_t i = 0; i < neu->Nv; i++) out[i] = 0.0;
+        /* an old leaf at the same level or above covers the new leaf: its (constant) value is the average */
+        int done = 0;
+        for (int ll = l; ll >= 0 && !done; ll--) {
+            const int sh = l - ll;
+            if (find_leaf(old, ll, c[0] >> sh, c[1] >> sh, c[2] >> sh) >= 0) {
+                int rc = remap_add(old, f_old, ll, c[0] >> sh, c[1] >> sh, c[2] >> sh, 1.0, out);
+                if (rc) {
+#pragma omp atomic write
+                    bad = rc;
+                }
+                done = 1;
+            }
+        }
+        /* otherwise the old leaves inside the new one, each with its volume fraction */
+        if (!done) {
+            int rc = remap_add(old, f_old, l, c[0], c[1], c[2], 1.0, out);
+            if (rc) {
+#pragma omp atomic write
+                bad = rc;
+            }
+        }
+    }
+    return bad;
+}
+
 /* face neighbours of one leaf (mesh query used to cut windows): returns count (<= 24) */
 int oracle_dvm_leaf_neighbours(const oracle_t *o, int64_t leaf, int64_t *ids) {
     int cnt = 0;

@@ -38,6 +38,8 @@ def lib():
         L.oracle_dvm_boundary_counts.argtypes = [C.c_void_p, C.c_void_p]
         L.oracle_dvm_leaf_neighbours.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
         L.oracle_dvm_kinetic_leaves.argtypes = [C.c_void_p, C.c_void_p]
+        L.oracle_dvm_remap.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.oracle_dvm_set_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -137,6 +139,16 @@ class Oracle:
             k = lib().oracle_dvm_leaf_neighbours(self._h, int(j), buf.ctypes.data)
             out.extend(buf[:k].tolist())
         return np.array(out, dtype=np.int64)
+
+    def remap_from(self, old: "Oracle", f_old):
+        """f on this mesh from f on `old` (volume average of the old piecewise-constant field, reading G20)."""
+        f_old = np.ascontiguousarray(f_old, np.float64)
+        assert f_old.shape == (old.n_kinetic, old.Nv)
+        out = np.empty((self.n_kinetic, self.Nv))
+        rc = lib().oracle_dvm_remap(old._h, self._h, f_old.ctypes.data, out.ctypes.data)
+        if rc != 0:
+            raise OracleError(rc, "remap: a new kinetic leaf lies over a SOLID leaf or outside the old mesh")
+        return out
 
     def kinetic_leaves(self):
         a = np.empty(self.n_kinetic, np.int64)
