@@ -86,7 +86,7 @@ def test_refine_then_coarsen_is_the_identity_to_roundoff():
     # injection: every fine leaf carries exactly its coarse ancestor's values
     assert set(np.unique(up[:, 0]).tolist()) <= set(f[:, 0].tolist())
     back = oc.remap_from(of, up)                       # mean of equal values: the identity to round-off
-    assert np.abs(back - f).max() <= 1e-15 * np.abs(f).max()
+    assert np.abs(back - f).max() <= 1e-14 * np.abs(f).max()       # up to 512 equal terms summed in sequence
 
 
 def test_uniform_state_stays_uniform():
