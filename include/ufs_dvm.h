@@ -136,6 +136,29 @@ int ufs_dvm_boundary_faces(ufs_dvm_t h, int64_t *n_faces, int64_t *cell, int8_t 
 int ufs_dvm_run_host(ufs_dvm_t h, const void *f_host_in, void *f_host_out, double *mom_dev_scratch,
                      double *mom_host, double dt, int nsteps);
 
+/* Mesh change on the device (the arrays of f and of the stencil records "are redone each time the
+ * spatial mesh is changed"; PAPER.md:199 names host preparation and transfer as the bottleneck).  Creates the handle of
+ * the new mesh exactly like ufs_dvm_create (new_desc, f_new_dev[2], cuda_stream, *out: same meaning, same errors) and
+ * fills f_new_dev[0] from the old handle's current f without leaving the device: an unchanged leaf keeps its f, a leaf
+ * created by refinement takes the f of the old leaf that covers it, a leaf created by coarsening the volume-weighted
+ * mean of the old leaves inside it (the volume average of the old piecewise-constant field: conservative, first
+ * order like the scheme), and a KINETIC leaf over an old FLUID leaf the Maxwellian of that leaf's frozen moments
+ * (PAPER.md:207).  Any refinement depth; velocity grid and storage type must not change (EINVAL); a new KINETIC leaf
+ * over an old SOLID leaf is EINVAL.  f_new_dev[0] must differ from the old handle's current buffer; f_new_dev[1] may
+ * be any buffer of the right size, e.g. the old handle's other one if it is large enough.  counts (HOST, may be
+ * NULL): new kinetic leaves copied / refined / coarsened, and sources that were FLUID leaves.  Synchronises the
+ * stream before returning; the old handle stays valid (destroy it when done).  On error *out may hold a handle whose
+ * ufs_dvm_last_error explains; destroy it. */
+int ufs_dvm_remesh(ufs_dvm_t old_handle, const ufs_dvm_desc *new_desc, void *f_new_dev[2], void *cuda_stream,
+                   ufs_dvm_t *out, int64_t counts[4]);
+
+/* The map ufs_dvm_remesh applies, for two existing handles (host-only handles will do; HOST outputs, NULL arrays for
+ * the sizes): new slab s = sum over k in [off[s], off[s+1]) of wgt[k] * source src[k], a source being slab src[k] of
+ * the old mesh if src[k] >= 0, else the frozen Maxwellian of the old FLUID leaf ghost_leaf[-1 - src[k]].
+ * off has n_kinetic(new) + 1 entries.  Errors are reported on new_handle. */
+int ufs_dvm_remap_plan(ufs_dvm_t old_handle, ufs_dvm_t new_handle, int64_t *n_entries, int64_t *off, int32_t *src,
+                       double *wgt, int64_t *n_ghosts, int64_t *ghost_leaf);
+
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
  * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes (bit 31: inflow ghost table, else

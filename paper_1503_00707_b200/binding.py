@@ -20,7 +20,7 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
-           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles"]
+           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -60,6 +60,8 @@ def lib() -> C.CDLL:
         L.ufs_dvm_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp]
         L.ufs_dvm_boundary_faces.argtypes = [vp, C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
         L.ufs_dvm_run_host.argtypes = [vp, vp, vp, vp, vp, C.c_double, C.c_int]
+        L.ufs_dvm_remesh.argtypes = [vp, C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p), vp]
+        L.ufs_dvm_remap_plan.argtypes = [vp, vp, C.POINTER(C.c_int64), vp, vp, vp, C.POINTER(C.c_int64), vp]
         L.ufs_dvm_tiles.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int32), vp, vp, vp, vp, C.POINTER(C.c_int64), vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
@@ -183,6 +185,30 @@ def ufs_dvm_boundary_faces(h):
     return cell, axis, side, area, kind, state
 
 
+def ufs_dvm_remesh(old_h, desc: ufs_dvm_desc, f_dev_ptrs, cuda_stream: int = 0):
+    """(new handle, counts[4]: copied, refined, coarsened, from-fluid)."""
+    h = C.c_void_p()
+    arr = (C.c_void_p * 2)(f_dev_ptrs[0], f_dev_ptrs[1])
+    counts = np.zeros(4, np.int64)
+    rc = lib().ufs_dvm_remesh(old_h, C.byref(desc), arr, C.c_void_p(cuda_stream), C.byref(h), counts.ctypes.data)
+    if rc != OK:
+        msg = lib().ufs_dvm_last_error(h).decode() if h else ""
+        lib().ufs_dvm_destroy(h)
+        raise UfsDvmError(rc, msg)
+    return h, counts
+
+
+def ufs_dvm_remap_plan(old_h, new_h, n_new_kinetic: int):
+    """(off, src, wgt, ghost_leaf) of the mesh-change map from old_h's mesh to new_h's (see include/ufs_dvm.h)."""
+    n, ng = C.c_int64(), C.c_int64()
+    _check(new_h, lib().ufs_dvm_remap_plan(old_h, new_h, C.byref(n), None, None, None, C.byref(ng), None))
+    off = np.zeros(n_new_kinetic + 1, np.int64); src = np.zeros(n.value, np.int32); wgt = np.zeros(n.value)
+    gl = np.zeros(ng.value, np.int64)
+    _check(new_h, lib().ufs_dvm_remap_plan(old_h, new_h, C.byref(n), off.ctypes.data, src.ctypes.data, wgt.ctypes.data,
+                                           C.byref(ng), gl.ctypes.data))
+    return off, src, wgt, gl
+
+
 def ufs_dvm_tiles(h) -> dict:
     """The flattener's tile records (see include/ufs_dvm.h); empty arrays if the handle uses another kernel."""
     n, pmax, ng = C.c_int64(), C.c_int32(), C.c_int64()
@@ -231,7 +257,9 @@ class DvmStepper:
     library's slab / slot order (ufs_dvm_layout) is applied here, on the host, with numpy."""
 
     def __init__(self, case: Case, device="cuda:0", kn: Optional[float] = None, storage: Optional[int] = None,
-                 stream=None):
+                 stream=None, remesh_from: Optional["DvmStepper"] = None):
+        """With `remesh_from`, the handle is made by ufs_dvm_remesh: f starts as the old stepper's current f carried
+        over to this case's mesh on the device (self.remesh_counts: copied, refined, coarsened, from-fluid)."""
         import torch
         self.torch = torch
         self.case = case
@@ -245,7 +273,11 @@ class DvmStepper:
             self.f = [torch.empty((n_kin, self.Nv), dtype=self.dtype, device=self.device) for _ in range(2)]
             self.mom = torch.empty((5, n_kin), dtype=torch.float64, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self.h = ufs_dvm_create(desc, [t.data_ptr() for t in self.f], self.stream.cuda_stream)
+            if remesh_from is None:
+                self.h = ufs_dvm_create(desc, [t.data_ptr() for t in self.f], self.stream.cuda_stream)
+            else:
+                self.h, self.remesh_counts = ufs_dvm_remesh(remesh_from.h, desc, [t.data_ptr() for t in self.f],
+                                                            self.stream.cuda_stream)
         self.n_kinetic, self.cell_of_slab, self.vel_of_slot = ufs_dvm_layout(self.h, self.Nv)
         assert self.n_kinetic == n_kin
         kin = case.kinetic_leaves()

@@ -434,6 +434,72 @@ int ufs_dvm_tiles(ufs_dvm_t h, int64_t* n_tiles, int32_t* pmax, int32_t* hdr, ui
     return UFS_DVM_OK;
 }
 
+int ufs_dvm_remap_plan(ufs_dvm_t old_h, ufs_dvm_t new_h, int64_t* n_entries, int64_t* off, int32_t* src, double* wgt,
+                       int64_t* n_ghosts, int64_t* ghost_leaf) {
+    if (!old_h || !new_h) return UFS_DVM_EINVAL;
+    RemapPlan plan;
+    std::string err;
+    const int rc = build_remap(old_h->mesh, new_h->mesh, plan, err);
+    if (rc) return fail(new_h, rc, err);
+    if (n_entries) *n_entries = (int64_t)plan.src.size();
+    if (off) std::memcpy(off, plan.off.data(), plan.off.size() * 8);
+    if (src) std::memcpy(src, plan.src.data(), plan.src.size() * 4);
+    if (wgt) std::memcpy(wgt, plan.wgt.data(), plan.wgt.size() * 8);
+    if (n_ghosts) *n_ghosts = (int64_t)plan.ghost_leaf.size();
+    if (ghost_leaf) std::memcpy(ghost_leaf, plan.ghost_leaf.data(), plan.ghost_leaf.size() * 8);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_remesh(ufs_dvm_t old_h, const ufs_dvm_desc* new_desc, void* f_new_dev[2], void* cuda_stream, ufs_dvm_t* out,
+                   int64_t counts[4]) {
+    if (!out) return UFS_DVM_EINVAL;
+    *out = nullptr;
+    if (!old_h || !old_h->device) return UFS_DVM_EINVAL;
+    if (old_h->sticky) return old_h->sticky;
+    int rc = ufs_dvm_create(new_desc, f_new_dev, cuda_stream, out);
+    if (rc) return rc;
+    ufs_dvm_t h = *out;   // errors below are reported on the new handle
+    if (h->storage != old_h->storage) return fail(h, UFS_DVM_EINVAL, "mesh change: the storage type must not change");
+    for (int b = 0; b < 2; b++)
+        if (h->mesh.n_kin > 0 && f_new_dev[0] == old_h->f[old_h->cur])
+            return fail(h, UFS_DVM_EINVAL, "mesh change: f_new_dev[0] must not be the old handle's current buffer");
+    RemapPlan plan;
+    try {
+        std::string err;
+        rc = build_remap(old_h->mesh, h->mesh, plan, err);
+        if (rc) return fail(h, rc, err);
+    } catch (const std::bad_alloc&) {
+        return fail(h, UFS_DVM_ENOMEM, "out of host memory while building the mesh-change map");
+    }
+    if (counts) { counts[0] = plan.n_copy; counts[1] = plan.n_prolong; counts[2] = plan.n_restrict; counts[3] = plan.n_from_fluid; }
+    if (h->mesh.n_kin == 0) return UFS_DVM_OK;
+    // the old handle's stream may differ: order the map after everything it has enqueued
+    if (old_h->stream != h->stream) {
+        cudaEvent_t ev;
+        CU(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "create event");
+        CU(cudaEventRecord(ev, old_h->stream), "record event");
+        CU(cudaStreamWaitEvent(h->stream, ev, 0), "wait event");
+        CU(cudaEventDestroy(ev), "destroy event");
+    }
+    int64_t* d_off = nullptr; int32_t* d_src = nullptr; double* d_wgt = nullptr; FluidGhost* d_gh = nullptr;
+    if ((rc = upload(h, &d_off, plan.off.data(), plan.off.size() * 8, "upload remap offsets"))) return rc;
+    if ((rc = upload(h, &d_src, plan.src.data(), plan.src.size() * 4, "upload remap sources"))) return rc;
+    if ((rc = upload(h, &d_wgt, plan.wgt.data(), plan.wgt.size() * 8, "upload remap weights"))) return rc;
+    if ((rc = upload(h, &d_gh, plan.ghosts.data(), plan.ghosts.size() * sizeof(FluidGhost), "upload remap ghosts"))) return rc;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev), "get device");
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "query SM count");
+    CU(launch_remap(h->storage, old_h->f[old_h->cur], h->f[0], d_off, d_src, d_wgt, d_gh, h->d_slot_k, h->mesh.n_kin, h->mesh.vel.Nv, sms, h->stream),
+       "remap kernel launch");
+    h->launches++;
+    h->cur = 0;
+    h->sums_valid = false;
+    // the map is read by that one launch only (the host vectors of `plan` die at return: wait for the uploads too)
+    CU(cudaStreamSynchronize(h->stream), "mesh change");
+    cudaFree(d_off); cudaFree(d_src); cudaFree(d_wgt); cudaFree(d_gh);
+    return UFS_DVM_OK;
+}
+
 int64_t ufs_dvm_launch_count(ufs_dvm_t h) { return h ? h->launches : 0; }
 
 int ufs_dvm_profile(ufs_dvm_t h, int enable) {

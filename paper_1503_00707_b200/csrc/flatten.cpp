@@ -385,6 +385,12 @@ int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
     }
     if (!ok) { err = "internal: a kinetic cell has a direction with neither 1 nor 4 sources"; return UFS_DVM_EMESH; }
 
+    // ---- the leaf list and its sorted keys stay with the mesh (mesh changes: build_remap) ----
+    m.leaf_level.assign(d.level, d.level + n);
+    m.leaf_kind.assign(d.kind, d.kind + n);
+    if (d.fluid_moments) m.leaf_fluid.assign(d.fluid_moments, d.fluid_moments + 5 * n);
+    m.start_keys = t.start;
+
     // ---- sibling octets among the slabs (tiles): eight consecutive slabs that are the children 0..7 of one parent ----
     m.octet_start.assign(m.n_kin, 0);
     for (int64_t s = 0; s + 7 < m.n_kin; s++) {
@@ -462,6 +468,61 @@ bool make_tile(const FlatMesh& m, int64_t s0, int nc, int pmax, TileBuild& t) {
 }
 
 }  // namespace
+
+int build_remap(const FlatMesh& o, const FlatMesh& nw, RemapPlan& plan, std::string& err) {
+    for (int a = 0; a < 3; a++)
+        if (o.vel.nv[a] != nw.vel.nv[a] || o.vel.xi[a][0] != nw.vel.xi[a][0] || o.vel.xi[a][o.vel.nv[a] - 1] != nw.vel.xi[a][o.vel.nv[a] - 1]) {
+            err = "mesh change: the two meshes must carry the same velocity grid";
+            return UFS_DVM_EINVAL;
+        }
+    const int LM = std::max(o.lmax, nw.lmax);               // common key depth
+    const int sh_o = 3 * (LM - o.lmax), sh_n = 3 * (LM - nw.lmax);
+    plan = RemapPlan{};
+    plan.off.assign(nw.n_kin + 1, 0);
+    std::vector<int64_t> ghost_of_leaf;
+    for (int64_t s = 0; s < nw.n_kin; s++) {
+        const int64_t j = nw.cell_of_slab[s];
+        const uint64_t k0 = nw.start_keys[nw.rank[j]] << sh_n;
+        const uint64_t size = 1ULL << (3 * (LM - nw.leaf_level[j]));
+        // first old leaf whose key interval contains k0
+        auto it = std::upper_bound(o.start_keys.begin(), o.start_keys.end(), k0 >> sh_o);
+        int64_t r = (it - o.start_keys.begin()) - 1;
+        int nsrc = 0;
+        while (r < o.n_leaves && (o.start_keys[r] << sh_o) < k0 + size) {
+            const int64_t q = o.order[r];
+            const uint64_t qsize = 1ULL << (3 * (LM - o.leaf_level[q]));
+            int32_t code;
+            if (o.leaf_kind[q] == UFS_CELL_KINETIC) {
+                code = (int32_t)o.slab_of_leaf[q];
+            } else if (o.leaf_kind[q] == UFS_CELL_FLUID) {
+                if (ghost_of_leaf.empty()) ghost_of_leaf.assign(o.n_leaves, -1);
+                if (ghost_of_leaf[q] < 0) {
+                    ghost_of_leaf[q] = (int64_t)plan.ghosts.size();
+                    plan.ghosts.emplace_back();
+                    plan.ghost_leaf.push_back(q);
+                    maxwell_factors(o.leaf_fluid.data() + 5 * q, o.vel, plan.ghosts.back());
+                }
+                code = (int32_t)(-1 - ghost_of_leaf[q]);
+                plan.n_from_fluid++;
+            } else {
+                err = "mesh change: a new KINETIC leaf lies over a SOLID leaf of the old mesh";
+                return UFS_DVM_EINVAL;
+            }
+            plan.src.push_back(code);
+            plan.wgt.push_back(qsize >= size ? 1.0 : (double)qsize / (double)size);
+            nsrc++;
+            if (qsize >= size) break;   // one old leaf covers the new one
+            r++;
+        }
+        if (nsrc == 0) { err = "mesh change: internal: no source for a new leaf"; return UFS_DVM_EMESH; }
+        const int64_t q0 = o.order[(it - o.start_keys.begin()) - 1];
+        if (nsrc > 1) plan.n_restrict++;
+        else if (o.leaf_level[q0] == nw.leaf_level[j]) plan.n_copy++;
+        else plan.n_prolong++;
+        plan.off[s + 1] = (int64_t)plan.src.size();
+    }
+    return UFS_DVM_OK;
+}
 
 void build_tiles(FlatMesh& m, int pmax) {
     m.tile_pmax = pmax;

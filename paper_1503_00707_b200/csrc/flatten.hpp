@@ -110,6 +110,10 @@ struct FlatMesh {
     std::vector<double> tables;         // [n_tables][Nv] inflow Maxwellians, SLOT order, fp64
     int64_t n_simple = 0;
     VelLayout vel;
+    // the leaf list itself and its Morton start keys (depth lmax), kept for mesh changes (build_remap)
+    std::vector<uint8_t> leaf_level, leaf_kind;
+    std::vector<double> leaf_fluid;         // [n_leaves][5] or empty
+    std::vector<uint64_t> start_keys;       // [n_leaves] Morton-sorted (position r = leaf order[r])
     // tiles (filled by build_tiles)
     std::vector<uint8_t> octet_start;       // [n_kin] 1: slabs s..s+7 are the eight leaf children of one parent, all kinetic
     int tile_pmax = 0;                      // piece-list stride
@@ -121,6 +125,20 @@ struct FlatMesh {
 
 // Returns UFS_DVM_OK or an error code with a message in `err`.
 int flatten(const ufs_dvm_desc& d, FlatMesh& out, std::string& err);
+
+// Mesh change (reading G20): every slab of the new mesh as a weighted sum of sources of
+// the old one -- one source of weight 1 where an old leaf covers the new one (unchanged leaf, or refinement: injection),
+// the old leaves inside it with their volume fractions where the new leaf is coarser (restriction).  A source is an old
+// slab (src >= 0) or the frozen Maxwellian of an old FLUID leaf (src = -1 - ghost index).
+struct RemapPlan {
+    std::vector<int64_t> off;          // [n_new_kin + 1]
+    std::vector<int32_t> src;
+    std::vector<double> wgt;
+    std::vector<FluidGhost> ghosts;    // factors of the old FLUID leaves that became KINETIC
+    std::vector<int64_t> ghost_leaf;   // ... and which old leaves they are
+    int64_t n_copy = 0, n_prolong = 0, n_restrict = 0, n_from_fluid = 0;
+};
+int build_remap(const FlatMesh& old_mesh, const FlatMesh& new_mesh, RemapPlan& plan, std::string& err);
 
 // Groups the slabs into tiles whose piece lists hold at most `pmax` pieces per octant (complete sibling octets where
 // the mesh has them, else runs of consecutive slabs) and fills the tile arrays of `m`.

@@ -89,6 +89,10 @@ bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan,
 cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 
+// remap.cu: f of a new mesh from f of the old one (weighted sums of old slabs / frozen fluid Maxwellians)
+cudaError_t launch_remap(int storage, const void* f_old, void* f_new, const int64_t* off, const int32_t* src, const double* wgt,
+                         const FluidGhost* ghosts, const uchar4* slot_k, int64_t n_new, int64_t Nv, int sm_count, cudaStream_t stream);
+
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 
