@@ -418,3 +418,24 @@ def morton_order(level: np.ndarray, ijk: np.ndarray) -> np.ndarray:
         for a in range(3):
             key |= ((xyz[:, a] >> b) & 1) << (3 * b + a)
     return np.argsort(key * 32 + level, kind="stable")
+
+
+def with_body_of(old: Case, new: Case, name: Optional[str] = None) -> Case:
+    """`new` with the solid body of `old`: every leaf of `new` that lies inside a SOLID leaf of `old` is SOLID (a mesh
+    change does not move the body; a staircase body re-sampled on a finer mesh would otherwise uncover KINETIC leaves
+    that have no old state to take over).  New SOLID leaves outside the old body are kept."""
+    import copy
+    solid = old.kind == CELL_SOLID
+    keys = {(int(l), int(i), int(j), int(k)) for l, (i, j, k) in zip(old.level[solid], old.ijk[solid])}
+    levels = sorted({k[0] for k in keys})
+    out = copy.copy(new)
+    out.kind = new.kind.copy()
+    for lo in levels:
+        m = new.level >= lo
+        sh = (new.level[m].astype(np.int64) - lo)[:, None]
+        anc = new.ijk[m].astype(np.int64) >> sh
+        hit = np.fromiter(((lo, int(a), int(b), int(c)) in keys for a, b, c in anc), bool, count=anc.shape[0])
+        idx = np.nonzero(m)[0][hit]
+        out.kind[idx] = CELL_SOLID
+    out.name = name or (new.name + "_body_of_" + old.name)
+    return out

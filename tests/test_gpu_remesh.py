@@ -111,10 +111,13 @@ def test_remesh_refuses_other_velocity_grid_and_solid_sources():
 
 
 def test_remesh_config3_to_config3_l8_at_stated_size():
-    """26 312 -> 154 188 kinetic leaves (sphere octree refined one more level around the body), fp64, after 3 steps on
-    the coarse mesh; the whole new field against the oracle's remap of the device's old field."""
+    """26 312 -> 152 240 kinetic leaves (sphere octree refined one more level around the body; the body itself is the
+    old mesh's staircase, inputs.with_body_of: the l_max 8 sampling of the sphere would uncover 1948 leaves inside old
+    SOLID leaves, which a mesh change refuses), fp64, after 3 steps on the coarse mesh; the whole new field against the
+    oracle's remap of the device's old field."""
     import torch
-    old, new = inputs.config3(lmax=7), inputs.config3(lmax=8)
+    old = inputs.config3(lmax=7)
+    new = inputs.with_body_of(old, inputs.config3(lmax=8))
     st_old = B.DvmStepper(old)
     harness.fill_initial_f_device(st_old, old)
     st_old.step(old.dt, 3)

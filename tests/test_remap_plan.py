@@ -84,3 +84,27 @@ def test_solid_source_is_refused():
         B.ufs_dvm_remap_plan(ho, hn, new.n_leaves)
     assert e.value.code == B.EINVAL and "SOLID" in str(e.value)
     B.ufs_dvm_destroy(ho); B.ufs_dvm_destroy(hn)
+
+
+def test_config3_to_l8_with_the_old_body_is_a_pure_refinement_map():
+    """The stated-size mesh change of tests/test_gpu_remesh.py, host side: with the old staircase body kept
+    (inputs.with_body_of) every new kinetic leaf has exactly one source of weight one; without it the map is refused
+    because the finer sampling of the sphere uncovers leaves inside old SOLID leaves."""
+    old, fine = inputs.config3(lmax=7), inputs.config3(lmax=8)
+    new = inputs.with_body_of(old, fine)
+    assert (new.kind == inputs.CELL_SOLID).sum() > (fine.kind == inputs.CELL_SOLID).sum()
+    ho = B.ufs_dvm_create_host(B.make_desc(old)[0])
+    try:
+        hn = B.ufs_dvm_create_host(B.make_desc(new)[0])
+        n_n, _, _ = B.ufs_dvm_layout(hn, new.Nv)
+        off, src, wgt, gl = B.ufs_dvm_remap_plan(ho, hn, n_n)
+        B.ufs_dvm_destroy(hn)
+        assert n_n == new.kinetic_leaves().size and np.all(np.diff(off) == 1)
+        assert np.all(wgt == 1.0) and np.all(src >= 0) and gl.size == 0
+        hf = B.ufs_dvm_create_host(B.make_desc(fine)[0])
+        with pytest.raises(B.UfsDvmError) as e:
+            B.ufs_dvm_remap_plan(ho, hf, fine.kinetic_leaves().size)
+        B.ufs_dvm_destroy(hf)
+        assert e.value.code == B.EINVAL and "SOLID" in str(e.value)
+    finally:
+        B.ufs_dvm_destroy(ho)
