@@ -32,6 +32,10 @@ constexpr int THX = 12;                 // values of a row (nh_x)
 constexpr int N_PROD = 4;               // producer warps: warps 0..3
 constexpr int N_CONS = 12;              // consumer warps: warps 4..15
 constexpr int NSTG = 8;                 // stage barrier pairs / stage descriptors
+// Register re-allocation between the warp groups (setmaxnreg): the CTA starts with 128 registers per thread (512 threads,
+// the whole file); the four producer warps give back down to REGS_PROD, the twelve consumer warps take REGS_CONS:
+// 4 * 32 * 80 + 12 * 32 * 144 = 65 536.
+constexpr int REGS_PROD = 80, REGS_CONS = 144;
 constexpr int TSLOTS = 3;               // tile header slots
 constexpr int DESC_BYTES = TILE_CELLS * CELLIDX_BYTES + 16;   // cell index tables, then the stage's first piece slot
 constexpr int THDR_NEXT = 36;           // tile header: TileHdr (32 B), tile id (or -1: stop), next tile id,
@@ -89,6 +93,7 @@ __device__ __forceinline__ void fluid_row_vec(const StepParams& p, int ghost, in
 template <typename T, bool FLUID, bool SUMS_ONLY>
 __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepParams p) {
     constexpr int VEC = V16<T>::N, RV = THX / VEC;
+    constexpr bool PACKED = sizeof(T) == 4 && !SUMS_ONLY;   // fp32 storage: packed two-value arithmetic in the row update
     constexpr uint32_t ROWB = THX * sizeof(T);          // bytes of a row
     constexpr uint32_t PB = NRP * ROWB;                 // bytes of a piece
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -120,6 +125,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
 
     if (warp < N_PROD) {
         // =========================================================== producer warps
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_PROD));
         const int w = warp;
         const T* fin = reinterpret_cast<const T*>(p.f_in);
         const int my_piece = 4 * lane + w;          // the piece of every stage this lane copies
@@ -244,6 +250,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
     }
 
     // =============================================================== consumer warps: thread = (cell c, row r of the piece)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_CONS));
     const int ct = tid - N_PROD * 32;
     const int c = ct / NRP, rr = ct % NRP;
     const int gi = rr >> 4;                          // 16-lane group of the cell
@@ -268,6 +275,15 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
         const double om1 = 1.0 - (double)omega, omd = om1 * dth;
         const T sxc = (T)omd;                         // times |xi_x,k| : the x coefficient
         const T cy = (T)(omd * ay);
+        // fp32 storage: the x coefficients of the row, Cx_k = sxc |xi_x,k|, as six packed pairs kept for the whole tile
+        float2 cx2[PACKED ? THX / 2 : 1];
+        if constexpr (PACKED) {
+#pragma unroll
+            for (int k = 0; k < THX / 2; k++) {
+                cx2[k] = make_float2(sxc * p.xf[2 * k], sxc * p.xf[2 * k + 1]);
+                asm volatile("" : "+f"(cx2[k].x), "+f"(cx2[k].y));   // kept in registers, not recomputed per stage
+            }
+        }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)(s0 + c) * p.Nv;
         double* const red = reinterpret_cast<double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)(c * 3 + gi) * SUMS_STRIDE;
         for (int q = 0; q < NQ; q++) {
@@ -275,6 +291,18 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
             const double az = p.vel->xi[2][p.nh[2] + rz];
             const T cz = (T)(omd * az);
             const T base = (T)(om1 - omd * (ay + az));
+            // ... and the own-value coefficients B - Cx_k:  f' = (B - Cx_k) f + Cx_k fX + Cy fY + Cz fZ + W gx_k
+            float2 bx2[PACKED ? THX / 2 : 1];
+            float2 cy2, cz2;
+            if constexpr (PACKED) {
+#pragma unroll
+                for (int k = 0; k < THX / 2; k++) {
+                    bx2[k] = make_float2(base - cx2[k].x, base - cx2[k].y);
+                    asm volatile("" : "+f"(bx2[k].x), "+f"(bx2[k].y));
+                }
+                cy2 = make_float2(cy, cy);
+                cz2 = make_float2(cz, cz);
+            }
             const int row = q * NRP + rr;             // row of the octant chunk
             // the 16 sign-weighted combinations of the row sums s_k = sum_x |xi_x|^k f' over the eight octants
             double E0 = 0, Ey = 0, Ez = 0, Eyz = 0, F0 = 0, Fx = 0, Fy = 0, Fxy = 0, Fz = 0, Fxz = 0, G0 = 0, Gx = 0, Gy = 0, Gz = 0, K0 = 0, Kx = 0;
@@ -300,6 +328,9 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     T wb = T(0);
                     const T* gxrow = tab + (o & 1) * nhp;
                     if (p.collide && !SUMS_ONLY) wb = omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rz] * tab[(2 + ((o >> 1) & 1)) * nhp + ry]);
+                    // packed path: the relaxation term is always added; with collisions off W = 0 multiplies the own row
+                    // (finite values) instead of a factor table nobody wrote
+                    const float* gxs = reinterpret_cast<const float*>(p.collide ? gxrow : a_own);
                     if (SUMS_ONLY) {
 #pragma unroll
                         for (int j = 0; j < RV; j++) {
@@ -327,16 +358,32 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             lds16(a_x + j * VEC, X);
                             lds16(a_y + j * VEC, Y);
                             lds16(a_z + j * VEC, Z);
+                            if constexpr (PACKED) {
+                                // two values per instruction (fma.rn.f32x2)
+                                const float2 wb2 = make_float2(wb, wb);
+                                float gx[4];
+                                lds16(gxs + j * 4, gx);
 #pragma unroll
-                            for (int i = 0; i < VEC; i++) {
-                                const T cx = sxc * tx_of<T>(p, j * VEC + i);
-                                out[i] = base * own[i] + cx * (X[i] - own[i]) + cy * Y[i] + cz * Z[i];
-                            }
-                            if (p.collide) {
-                                T gx[VEC];
-                                lds16(gxrow + j * VEC, gx);
+                                for (int h = 0; h < 2; h++) {
+                                    float2 m = __fmul2_rn(cx2[2 * j + h], make_float2(X[2 * h], X[2 * h + 1]));
+                                    m = __ffma2_rn(bx2[2 * j + h], make_float2(own[2 * h], own[2 * h + 1]), m);
+                                    m = __ffma2_rn(cy2, make_float2(Y[2 * h], Y[2 * h + 1]), m);
+                                    m = __ffma2_rn(cz2, make_float2(Z[2 * h], Z[2 * h + 1]), m);
+                                    m = __ffma2_rn(wb2, make_float2(gx[2 * h], gx[2 * h + 1]), m);
+                                    out[2 * h] = m.x; out[2 * h + 1] = m.y;
+                                }
+                            } else {
 #pragma unroll
-                                for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+                                for (int i = 0; i < VEC; i++) {
+                                    const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                    out[i] = base * own[i] + cx * (X[i] - own[i]) + cy * Y[i] + cz * Z[i];
+                                }
+                                if (p.collide) {
+                                    T gx[VEC];
+                                    lds16(gxrow + j * VEC, gx);
+#pragma unroll
+                                    for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+                                }
                             }
                             stg16_cs(gdst + j * VEC, out);
 #pragma unroll
