@@ -302,6 +302,13 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                 }
                 cy2 = make_float2(cy, cy);
                 cz2 = make_float2(cz, cz);
+                asm volatile("" : "+f"(cy2.x), "+f"(cy2.y), "+f"(cz2.x), "+f"(cz2.y));
+            }
+            // relaxation weights of the row for the two signs of xi_y and of xi_z: W = omega gz[sz][rz] gy[sy][ry]
+            T wgy[2] = {T(0), T(0)}, wgz[2] = {T(0), T(0)};
+            if (p.collide && !SUMS_ONLY) {
+                wgy[0] = omega * tab[2 * nhp + ry]; wgy[1] = omega * tab[3 * nhp + ry];
+                wgz[0] = tab[4 * nhp + rz];         wgz[1] = tab[5 * nhp + rz];
             }
             const int row = q * NRP + rr;             // row of the octant chunk
             // the 16 sign-weighted combinations of the row sums s_k = sum_x |xi_x|^k f' over the eight octants
@@ -327,7 +334,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX;
                     T wb = T(0);
                     const T* gxrow = tab + (o & 1) * nhp;
-                    if (p.collide && !SUMS_ONLY) wb = omega * (tab[(4 + ((o >> 2) & 1)) * nhp + rz] * tab[(2 + ((o >> 1) & 1)) * nhp + ry]);
+                    if (!SUMS_ONLY) wb = ((o & 4) ? wgz[1] : wgz[0]) * ((o & 2) ? wgy[1] : wgy[0]);
                     // packed path: the relaxation term is always added; with collisions off W = 0 multiplies the own row
                     // (finite values) instead of a factor table nobody wrote
                     const float* gxs = reinterpret_cast<const float*>(p.collide ? gxrow : a_own);
