@@ -159,6 +159,61 @@ int ufs_dvm_remesh(ufs_dvm_t old_handle, const ufs_dvm_desc *new_desc, void *f_n
 int ufs_dvm_remap_plan(ufs_dvm_t old_handle, ufs_dvm_t new_handle, int64_t *n_entries, int64_t *off, int32_t *src,
                        double *wgt, int64_t *n_ghosts, int64_t *ghost_leaf);
 
+/* ---- Partitioned mesh: one GPU (process) per rank (PAPER.md:57 space-filling-curve partition, Fig. 3; PAPER.md:185-187
+ * multi-GPU advection, Fig. 5: "inner cells are stored before ghost cells", ghost cells gathered before the kernel runs;
+ * the collision part is local).
+ *
+ * ufs_dvm_partition: rank_of_leaf[n_leaves] (HOST output).  The leaves in N-order (Morton), each weighted by its cost
+ * (w_kinetic for KINETIC, w_fluid for FLUID, 0 for SOLID leaves; "weight proportional to the CPU time"),
+ * are cut into n_ranks consecutive ranges of equal weight: every rank's weight is within one leaf's weight of the mean.
+ * No handle, no CUDA. */
+int ufs_dvm_partition(const ufs_dvm_desc *desc, int32_t n_ranks, double w_kinetic, double w_fluid,
+                      int32_t *rank_of_leaf);
+
+/* Rank my_rank's part of the WHOLE mesh `desc` (every rank passes the same desc and rank_of_leaf, HOST arrays read during
+ * the call only; any ownership whose KINETIC leaves form one N-order range per rank is accepted, EINVAL otherwise).  The
+ * handle steps the rank's own ("inner") KINETIC leaves; its slabs are the inner leaves in N-order followed by the ghost
+ * cells: KINETIC leaves of other ranks that are upwind sources of inner leaves.  f_dev[0], f_dev[1]: DEVICE buffers of
+ * (n_inner + n_ghost) * Nv elements (sizes: ufs_dvm_part_layout of the host-only variant); the caller fills the inner
+ * slabs of f_dev[0] (ufs_dvm_layout gives leaf and slot order), the ghost slabs arrive by the exchange below.
+ * Per step:   for every peer p:  ufs_dvm_halo_pack(h, p, send_p)  ->  transfer send_p to rank p's recv buffer for this
+ * rank (ncclSend / ncclRecv on the handle's stream, or any copy)  ->  ufs_dvm_halo_unpack(h, p, recv_p);   then
+ * ufs_dvm_halo_done(h);  ufs_dvm_step(h, dt, 1).   A step without fresh ghosts, or nsteps > 1, is EINVAL.  Needs the
+ * octant layout (even, symmetric velocity grid).  ufs_dvm_moments / ufs_dvm_layout describe the inner leaves only;
+ * ufs_dvm_run_host, ufs_dvm_remesh and ufs_dvm_remap_plan refuse a partitioned handle. */
+int ufs_dvm_create_part(const ufs_dvm_desc *desc, const int32_t *rank_of_leaf, int32_t my_rank, int32_t n_ranks,
+                        void *f_dev[2], void *cuda_stream, ufs_dvm_t *out);
+int ufs_dvm_create_part_host(const ufs_dvm_desc *desc, const int32_t *rank_of_leaf, int32_t my_rank,
+                             int32_t n_ranks, ufs_dvm_t *out);
+
+/* Slab layout of a partitioned handle (HOST outputs, any may be NULL): *n_inner, *n_ghost, *first_global_slab (inner slab
+ * s is slab first_global_slab + s of the unpartitioned mesh), leaf_of_slab[n_inner + n_ghost] (leaf-list indices),
+ * owner_of_ghost[n_ghost].  For an unpartitioned handle n_ghost = 0. */
+int ufs_dvm_part_layout(ufs_dvm_t h, int64_t *n_inner, int64_t *n_ghost, int64_t *first_global_slab,
+                        int64_t *leaf_of_slab, int32_t *owner_of_ghost);
+
+/* Halo lists towards rank `peer` (HOST outputs; NULL arrays for the counts): send_slab[n_send] inner slabs and
+ * send_mask[n_send] which of their 8 octant chunks (bit o: sign group o = sx + 2 sy + 4 sz, bit set if xi > 0) the peer
+ * needs; recv_slab[n_recv] ghost slabs and recv_mask[n_recv] the chunks that arrive from the peer.  Both lists ascend in
+ * the cell's slab number in the unpartitioned mesh, so the k-th entry sent is the k-th entry the peer receives.  Only the
+ * upwind chunks cross: for a face on axis a the four sign groups whose xi_a points from the ghost into the inner cell
+ * (PAPER.md:106-108). */
+int ufs_dvm_halo(ufs_dvm_t h, int32_t peer, int64_t *n_send, int32_t *send_slab, uint8_t *send_mask,
+                 int64_t *n_recv, int32_t *recv_slab, uint8_t *recv_mask);
+
+/* Sizes in bytes of the packed buffers exchanged with `peer` (HOST outputs): listed chunks x chunk size. */
+int ufs_dvm_halo_bytes(ufs_dvm_t h, int32_t peer, int64_t *send_bytes, int64_t *recv_bytes);
+
+/* Enqueue: gather the chunks of the send list of `peer` from the current f into buf_dev (DEVICE, 16-byte aligned,
+ * send_bytes), entries in list order, a slab's chunks by ascending octant / scatter buf_dev (recv_bytes) into the ghost
+ * slabs of the current f. */
+int ufs_dvm_halo_pack(ufs_dvm_t h, int32_t peer, void *buf_dev);
+int ufs_dvm_halo_unpack(ufs_dvm_t h, int32_t peer, const void *buf_dev);
+
+/* Every peer's chunks have been unpacked (enqueued on the handle's stream): enqueue the velocity sums of the ghost cells
+ * and allow the next ufs_dvm_step. */
+int ufs_dvm_halo_done(ufs_dvm_t h);
+
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
  * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes (bit 31: inflow ghost table, else

@@ -20,7 +20,9 @@ _CODES = {EINVAL: "EINVAL", EMESH: "EMESH", ECUDA: "ECUDA", ENOMEM: "ENOMEM", EN
 EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_moments", "ufs_dvm_sync",
            "ufs_dvm_destroy", "ufs_dvm_current", "ufs_dvm_layout", "ufs_dvm_faces", "ufs_dvm_boundary_faces",
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
-           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan"]
+           "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan",
+           "ufs_dvm_partition", "ufs_dvm_create_part", "ufs_dvm_create_part_host", "ufs_dvm_part_layout", "ufs_dvm_halo",
+           "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done"]
 
 
 class ufs_dvm_desc(C.Structure):
@@ -63,6 +65,16 @@ def lib() -> C.CDLL:
         L.ufs_dvm_remesh.argtypes = [vp, C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p), vp]
         L.ufs_dvm_remap_plan.argtypes = [vp, vp, C.POINTER(C.c_int64), vp, vp, vp, C.POINTER(C.c_int64), vp]
         L.ufs_dvm_tiles.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int32), vp, vp, vp, vp, C.POINTER(C.c_int64), vp]
+        i32p = C.c_void_p
+        L.ufs_dvm_partition.argtypes = [C.POINTER(ufs_dvm_desc), C.c_int32, C.c_double, C.c_double, i32p]
+        L.ufs_dvm_create_part.argtypes = [C.POINTER(ufs_dvm_desc), i32p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p)]
+        L.ufs_dvm_create_part_host.argtypes = [C.POINTER(ufs_dvm_desc), i32p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
+        L.ufs_dvm_part_layout.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp, vp]
+        L.ufs_dvm_halo.argtypes = [vp, C.c_int32, C.POINTER(C.c_int64), vp, vp, C.POINTER(C.c_int64), vp, vp]
+        L.ufs_dvm_halo_bytes.argtypes = [vp, C.c_int32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.ufs_dvm_halo_pack.argtypes = [vp, C.c_int32, vp]
+        L.ufs_dvm_halo_unpack.argtypes = [vp, C.c_int32, vp]
+        L.ufs_dvm_halo_done.argtypes = [vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
@@ -209,6 +221,75 @@ def ufs_dvm_remap_plan(old_h, new_h, n_new_kinetic: int):
     return off, src, wgt, gl
 
 
+def ufs_dvm_partition(desc: ufs_dvm_desc, n_ranks: int, w_kinetic: float = 1.0, w_fluid: float = 0.0) -> np.ndarray:
+    """rank_of_leaf[n_leaves] int32."""
+    out = np.empty(int(desc.n_leaves), np.int32)
+    rc = lib().ufs_dvm_partition(C.byref(desc), int(n_ranks), float(w_kinetic), float(w_fluid), out.ctypes.data)
+    if rc != OK:
+        raise UfsDvmError(rc, "ufs_dvm_partition")
+    return out
+
+
+def _created(rc, h):
+    if rc != OK:
+        msg = lib().ufs_dvm_last_error(h).decode() if h else ""
+        lib().ufs_dvm_destroy(h)
+        raise UfsDvmError(rc, msg)
+    return h
+
+
+def ufs_dvm_create_part_host(desc: ufs_dvm_desc, rank_of_leaf: np.ndarray, my_rank: int, n_ranks: int) -> C.c_void_p:
+    h = C.c_void_p()
+    rol = np.ascontiguousarray(rank_of_leaf, np.int32)
+    return _created(lib().ufs_dvm_create_part_host(C.byref(desc), rol.ctypes.data, int(my_rank), int(n_ranks), C.byref(h)), h)
+
+
+def ufs_dvm_create_part(desc: ufs_dvm_desc, rank_of_leaf: np.ndarray, my_rank: int, n_ranks: int, f_dev_ptrs,
+                        cuda_stream: int = 0) -> C.c_void_p:
+    h = C.c_void_p()
+    rol = np.ascontiguousarray(rank_of_leaf, np.int32)
+    arr = (C.c_void_p * 2)(f_dev_ptrs[0], f_dev_ptrs[1])
+    return _created(lib().ufs_dvm_create_part(C.byref(desc), rol.ctypes.data, int(my_rank), int(n_ranks), arr,
+                                              C.c_void_p(cuda_stream), C.byref(h)), h)
+
+
+def ufs_dvm_part_layout(h) -> dict:
+    n_in, n_gh, g0 = C.c_int64(), C.c_int64(), C.c_int64()
+    _check(h, lib().ufs_dvm_part_layout(h, C.byref(n_in), C.byref(n_gh), C.byref(g0), None, None))
+    leaf = np.empty(n_in.value + n_gh.value, np.int64)
+    owner = np.empty(n_gh.value, np.int32)
+    _check(h, lib().ufs_dvm_part_layout(h, None, None, None, leaf.ctypes.data, owner.ctypes.data))
+    return {"n_inner": n_in.value, "n_ghost": n_gh.value, "first_global_slab": g0.value, "leaf_of_slab": leaf,
+            "owner_of_ghost": owner}
+
+
+def ufs_dvm_halo(h, peer: int) -> dict:
+    ns, nr = C.c_int64(), C.c_int64()
+    _check(h, lib().ufs_dvm_halo(h, int(peer), C.byref(ns), None, None, C.byref(nr), None, None))
+    ss, sm = np.empty(ns.value, np.int32), np.empty(ns.value, np.uint8)
+    rs, rm = np.empty(nr.value, np.int32), np.empty(nr.value, np.uint8)
+    _check(h, lib().ufs_dvm_halo(h, int(peer), None, ss.ctypes.data, sm.ctypes.data, None, rs.ctypes.data, rm.ctypes.data))
+    return {"send_slab": ss, "send_mask": sm, "recv_slab": rs, "recv_mask": rm}
+
+
+def ufs_dvm_halo_bytes(h, peer: int):
+    sb, rb = C.c_int64(), C.c_int64()
+    _check(h, lib().ufs_dvm_halo_bytes(h, int(peer), C.byref(sb), C.byref(rb)))
+    return sb.value, rb.value
+
+
+def ufs_dvm_halo_pack(h, peer: int, buf_dev_ptr: int):
+    _check(h, lib().ufs_dvm_halo_pack(h, int(peer), C.c_void_p(buf_dev_ptr)))
+
+
+def ufs_dvm_halo_unpack(h, peer: int, buf_dev_ptr: int):
+    _check(h, lib().ufs_dvm_halo_unpack(h, int(peer), C.c_void_p(buf_dev_ptr)))
+
+
+def ufs_dvm_halo_done(h):
+    _check(h, lib().ufs_dvm_halo_done(h))
+
+
 def ufs_dvm_tiles(h) -> dict:
     """The flattener's tile records (see include/ufs_dvm.h); empty arrays if the handle uses another kernel."""
     n, pmax, ng = C.c_int64(), C.c_int32(), C.c_int64()
@@ -295,9 +376,10 @@ class DvmStepper:
         slot_t = torch.as_tensor(self.vel_of_slot.astype(np.int64), device=self.device)
         with torch.cuda.stream(self.stream):     # the copies must be ordered with the handle's stream
             for s0 in range(0, self.n_kinetic, chunk):
-                rows = self.row_of_slab[s0:s0 + chunk]
+                s1 = min(s0 + chunk, self.n_kinetic)       # (a partitioned handle's tensors hold ghost slabs after these)
+                rows = self.row_of_slab[s0:s1]
                 part = torch.from_numpy(np.ascontiguousarray(f_rows[rows])).to(self.device)
-                self.f[cur][s0:s0 + chunk].copy_(part.index_select(1, slot_t).to(self.dtype))
+                self.f[cur][s0:s1].copy_(part.index_select(1, slot_t).to(self.dtype))
         ufs_dvm_f_changed(self.h)
 
     def read_canonical(self, slabs: Optional[np.ndarray] = None) -> np.ndarray:
@@ -318,8 +400,9 @@ class DvmStepper:
                 return out
             out = np.empty((self.n_kinetic, self.Nv))
             for s0 in range(0, self.n_kinetic, chunk):
-                part = self.f[cur][s0:s0 + chunk].index_select(1, inv_t).double().cpu().numpy()
-                out[self.row_of_slab[s0:s0 + chunk]] = part
+                s1 = min(s0 + chunk, self.n_kinetic)
+                part = self.f[cur][s0:s1].index_select(1, inv_t).double().cpu().numpy()
+                out[self.row_of_slab[s0:s1]] = part
         return out
 
     def step(self, dt: float, nsteps: int = 1):

@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/ufs_dvm.h"
 #include "flatten.hpp"
@@ -37,6 +38,10 @@ struct ufs_dvm_s {
     uint32_t* d_tile_pieces = nullptr;
     uint8_t* d_tile_cellidx = nullptr;
     int32_t* d_tile_fluid = nullptr;
+    // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
+    std::vector<int32_t*> d_send_chunks, d_recv_chunks;
+    std::vector<int64_t> n_send_chunks, n_recv_chunks;
+    bool ghosts_fresh = false;     // the ghost slabs of f[cur] and their sums are those of the peers' current f
     bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
     StepLaunch plan{};
@@ -139,7 +144,7 @@ void ghost_state_sums(const VelLayout& v, F value_of_slot, double* out) {
     }
 }
 
-int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out) {
+int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out, const int32_t* rank_of_leaf = nullptr, int my_rank = 0, int n_ranks = 1) {
     if (!out) return UFS_DVM_EINVAL;
     *out = nullptr;
     if (!desc) return UFS_DVM_EINVAL;
@@ -152,6 +157,11 @@ int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out) {
         std::string err;
         int rc = flatten(*desc, h->mesh, err);
         if (rc) return fail(h, rc, err);
+        if (rank_of_leaf) {
+            if (!h->mesh.vel.fast) return fail(h, UFS_DVM_EINVAL, "a partitioned mesh needs the octant layout (even, symmetric velocity grid)");
+            rc = restrict_to_rank(h->mesh, rank_of_leaf, my_rank, n_ranks, err);
+            if (rc) return fail(h, rc, err);
+        }
     } catch (const std::bad_alloc&) {
         return fail(h, UFS_DVM_ENOMEM, "out of host memory while flattening");
     } catch (...) {
@@ -190,10 +200,62 @@ extern "C" {
 
 int ufs_dvm_create_host(const ufs_dvm_desc* desc, ufs_dvm_t* out) { return create_common(desc, out); }
 
+static int create_device(ufs_dvm_t h, void* f_dev[2], void* cuda_stream);
+
 int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, ufs_dvm_t* out) {
     int rc = create_common(desc, out);
     if (rc) return rc;
+    return create_device(*out, f_dev, cuda_stream);
+}
+
+int ufs_dvm_partition(const ufs_dvm_desc* desc, int32_t n_ranks, double w_kinetic, double w_fluid, int32_t* rank_of_leaf) {
+    if (!desc) return UFS_DVM_EINVAL;
+    std::string err;
+    try {
+        return partition_leaves(*desc, n_ranks, w_kinetic, w_fluid, rank_of_leaf, err);
+    } catch (...) {
+        return UFS_DVM_ENOMEM;
+    }
+}
+
+int ufs_dvm_create_part_host(const ufs_dvm_desc* desc, const int32_t* rank_of_leaf, int32_t my_rank, int32_t n_ranks, ufs_dvm_t* out) {
+    if (!rank_of_leaf) { if (out) *out = nullptr; return UFS_DVM_EINVAL; }
+    return create_common(desc, out, rank_of_leaf, my_rank, n_ranks);
+}
+
+int ufs_dvm_create_part(const ufs_dvm_desc* desc, const int32_t* rank_of_leaf, int32_t my_rank, int32_t n_ranks, void* f_dev[2],
+                        void* cuda_stream, ufs_dvm_t* out) {
+    int rc = ufs_dvm_create_part_host(desc, rank_of_leaf, my_rank, n_ranks, out);
+    if (rc) return rc;
     ufs_dvm_t h = *out;
+    if ((rc = create_device(h, f_dev, cuda_stream))) return rc;
+    // the ghost slabs start finite (chunks that never arrive are never used, but their sums are formed)
+    const FlatMesh& m = h->mesh;
+    const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
+    const size_t off = (size_t)m.n_kin * m.vel.Nv * elem, len = (size_t)(m.n_slabs - m.n_kin) * m.vel.Nv * elem;
+    if (len)
+        for (int b = 0; b < 2; b++) CU(cudaMemsetAsync(static_cast<char*>(h->f[b]) + off, 0, len, h->stream), "clear ghost slabs");
+    // chunk lists per peer
+    h->d_send_chunks.assign(m.n_ranks, nullptr); h->d_recv_chunks.assign(m.n_ranks, nullptr);
+    h->n_send_chunks.assign(m.n_ranks, 0); h->n_recv_chunks.assign(m.n_ranks, 0);
+    for (int pr = 0; pr < m.n_ranks; pr++)
+        for (int dir = 0; dir < 2; dir++) {
+            const std::vector<int32_t>& slab = dir ? m.recv_slab[pr] : m.send_slab[pr];
+            const std::vector<uint8_t>& mask = dir ? m.recv_mask[pr] : m.send_mask[pr];
+            std::vector<int32_t> chunks;
+            for (size_t i = 0; i < slab.size(); i++)
+                for (int o = 0; o < 8; o++)
+                    if (mask[i] & (1u << o)) chunks.push_back(slab[i] * 8 + o);
+            (dir ? h->n_recv_chunks : h->n_send_chunks)[pr] = (int64_t)chunks.size();
+            if ((rc = upload(h, dir ? &h->d_recv_chunks[pr] : &h->d_send_chunks[pr], chunks.data(), chunks.size() * 4, "upload halo chunk lists"))) return rc;
+            CU(cudaStreamSynchronize(h->stream), "upload");   // `chunks` dies here
+        }
+    h->ghosts_fresh = m.n_slabs == m.n_kin;
+    return UFS_DVM_OK;
+}
+
+static int create_device(ufs_dvm_t h, void* f_dev[2], void* cuda_stream) {
+    int rc = UFS_DVM_OK;
     if (!f_dev || ((!f_dev[0] || !f_dev[1]) && h->mesh.n_kin > 0)) return fail(h, UFS_DVM_EINVAL, "f_dev[0] and f_dev[1] must be device buffers");
     if (h->mesh.n_kin > 0 && (f_dev[0] == f_dev[1] || ((uintptr_t)f_dev[0] & 15) || ((uintptr_t)f_dev[1] & 15)))
         return fail(h, UFS_DVM_EINVAL, "the two f buffers must be distinct and 16-byte aligned");
@@ -240,7 +302,7 @@ int ufs_dvm_create(const ufs_dvm_desc* desc, void* f_dev[2], void* cuda_stream, 
     }
     if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
-        const size_t sums_bytes = (size_t)m.n_kin * SUMS_STRIDE * sizeof(double);
+        const size_t sums_bytes = (size_t)m.n_slabs * SUMS_STRIDE * sizeof(double);   // ghost cells carry sums too
         for (int b = 0; b < 2; b++) CU(cudaMalloc(reinterpret_cast<void**>(&h->d_sums[b]), sums_bytes), "allocate velocity sums");
         CU(cudaMalloc(&h->d_tabs, (size_t)m.n_kin * stream_tabn(v) * elem), "allocate factor tables");
         // sums of the ghost states (inflow tables, fluid leaves), from the values the kernel will read
@@ -285,6 +347,10 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!(dt > 0) || nsteps < 0) return fail(h, UFS_DVM_EINVAL, "dt must be positive and nsteps >= 0");
+    const bool has_ghosts = h->mesh.n_slabs > h->mesh.n_kin;
+    if (has_ghosts && nsteps > 1) return fail(h, UFS_DVM_EINVAL, "a partitioned mesh is stepped one step at a time (ghost exchange in between)");
+    if (has_ghosts && nsteps == 1 && !h->ghosts_fresh)
+        return fail(h, UFS_DVM_EINVAL, "ghost cells are stale: exchange them (ufs_dvm_halo_pack / unpack) and call ufs_dvm_halo_done before the step");
     const bool stream = h->plan.ring >= 2 && h->mesh.n_kin > 0;
     for (int s = 0; s < nsteps; s++) {
         if (stream && !h->sums_valid) {
@@ -304,6 +370,7 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
         CU(launch_step(h->storage, plan, p, h->stream), "step kernel launch");
         h->cur ^= 1;
         h->parity ^= 1;
+        if (has_ghosts) h->ghosts_fresh = false;
         if (h->mesh.n_kin > 0) h->launches += (stream && p.collide) ? 2 : 1;
     }
     return UFS_DVM_OK;
@@ -352,6 +419,8 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
         cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_tile_fluid);
+        for (int32_t* q : h->d_send_chunks) cudaFree(q);
+        for (int32_t* q : h->d_recv_chunks) cudaFree(q);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
     }
     delete h;
@@ -408,6 +477,7 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, doubl
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!f_host_in || !mom_dev_scratch || !mom_host) return fail(h, UFS_DVM_EINVAL, "NULL buffer");
+    if (h->mesh.partial) return fail(h, UFS_DVM_EINVAL, "ufs_dvm_run_host does not drive a partitioned mesh (ghost exchange between steps)");
     const size_t bytes = (size_t)h->mesh.n_kin * (size_t)h->mesh.vel.Nv * (h->storage == UFS_STORE_F32 ? 4 : 8);
     CU(cudaMemcpyAsync(h->f[h->cur], f_host_in, bytes, cudaMemcpyHostToDevice, h->stream), "copy f to the device");
     h->sums_valid = false;
@@ -437,6 +507,7 @@ int ufs_dvm_tiles(ufs_dvm_t h, int64_t* n_tiles, int32_t* pmax, int32_t* hdr, ui
 int ufs_dvm_remap_plan(ufs_dvm_t old_h, ufs_dvm_t new_h, int64_t* n_entries, int64_t* off, int32_t* src, double* wgt,
                        int64_t* n_ghosts, int64_t* ghost_leaf) {
     if (!old_h || !new_h) return UFS_DVM_EINVAL;
+    if (old_h->mesh.partial || new_h->mesh.partial) return fail(new_h, UFS_DVM_EINVAL, "mesh change of a partitioned mesh is not supported");
     RemapPlan plan;
     std::string err;
     const int rc = build_remap(old_h->mesh, new_h->mesh, plan, err);
@@ -456,6 +527,7 @@ int ufs_dvm_remesh(ufs_dvm_t old_h, const ufs_dvm_desc* new_desc, void* f_new_de
     *out = nullptr;
     if (!old_h || !old_h->device) return UFS_DVM_EINVAL;
     if (old_h->sticky) return old_h->sticky;
+    if (old_h->mesh.partial) return UFS_DVM_EINVAL;
     int rc = ufs_dvm_create(new_desc, f_new_dev, cuda_stream, out);
     if (rc) return rc;
     ufs_dvm_t h = *out;   // errors below are reported on the new handle
@@ -497,6 +569,85 @@ int ufs_dvm_remesh(ufs_dvm_t old_h, const ufs_dvm_desc* new_desc, void* f_new_de
     // the map is read by that one launch only (the host vectors of `plan` die at return: wait for the uploads too)
     CU(cudaStreamSynchronize(h->stream), "mesh change");
     cudaFree(d_off); cudaFree(d_src); cudaFree(d_wgt); cudaFree(d_gh);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_part_layout(ufs_dvm_t h, int64_t* n_inner, int64_t* n_ghost, int64_t* first_global_slab, int64_t* leaf_of_slab, int32_t* owner_of_ghost) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    if (n_inner) *n_inner = m.n_kin;
+    if (n_ghost) *n_ghost = m.n_slabs - m.n_kin;
+    if (first_global_slab) *first_global_slab = m.first_global_slab;
+    if (leaf_of_slab) std::memcpy(leaf_of_slab, m.cell_of_slab.data(), (size_t)m.n_slabs * 8);
+    if (owner_of_ghost && !m.ghost_owner.empty()) std::memcpy(owner_of_ghost, m.ghost_owner.data(), m.ghost_owner.size() * 4);
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_halo(ufs_dvm_t h, int32_t peer, int64_t* n_send, int32_t* send_slab, uint8_t* send_mask, int64_t* n_recv,
+                 int32_t* recv_slab, uint8_t* recv_mask) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    if (!m.partial || peer < 0 || peer >= m.n_ranks) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh, or no such peer");
+    if (n_send) *n_send = (int64_t)m.send_slab[peer].size();
+    if (n_recv) *n_recv = (int64_t)m.recv_slab[peer].size();
+    if (send_slab && !m.send_slab[peer].empty()) std::memcpy(send_slab, m.send_slab[peer].data(), m.send_slab[peer].size() * 4);
+    if (send_mask && !m.send_mask[peer].empty()) std::memcpy(send_mask, m.send_mask[peer].data(), m.send_mask[peer].size());
+    if (recv_slab && !m.recv_slab[peer].empty()) std::memcpy(recv_slab, m.recv_slab[peer].data(), m.recv_slab[peer].size() * 4);
+    if (recv_mask && !m.recv_mask[peer].empty()) std::memcpy(recv_mask, m.recv_mask[peer].data(), m.recv_mask[peer].size());
+    return UFS_DVM_OK;
+}
+
+static int64_t chunk_bytes_of(ufs_dvm_t h) {
+    const VelLayout& v = h->mesh.vel;
+    return (int64_t)v.nh[0] * v.nh[1] * v.nh[2] * (h->storage == UFS_STORE_F32 ? 4 : 8);
+}
+
+int ufs_dvm_halo_bytes(ufs_dvm_t h, int32_t peer, int64_t* send_bytes, int64_t* recv_bytes) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    if (!m.partial || peer < 0 || peer >= m.n_ranks) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh, or no such peer");
+    int64_t ns = 0, nr = 0;
+    for (uint8_t mk : m.send_mask[peer]) ns += __builtin_popcount(mk);
+    for (uint8_t mk : m.recv_mask[peer]) nr += __builtin_popcount(mk);
+    if (send_bytes) *send_bytes = ns * chunk_bytes_of(h);
+    if (recv_bytes) *recv_bytes = nr * chunk_bytes_of(h);
+    return UFS_DVM_OK;
+}
+
+static int halo_copy(ufs_dvm_t h, int32_t peer, void* buf, bool pack) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    const FlatMesh& m = h->mesh;
+    if (!m.partial || peer < 0 || peer >= m.n_ranks) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh, or no such peer");
+    const int64_t n = pack ? h->n_send_chunks[peer] : h->n_recv_chunks[peer];
+    if (n == 0) return UFS_DVM_OK;
+    if (!buf || ((uintptr_t)buf & 15)) return fail(h, UFS_DVM_EINVAL, "the halo buffer must be a 16-byte aligned device buffer");
+    CU(launch_halo_copy(pack, pack ? h->d_send_chunks[peer] : h->d_recv_chunks[peer], n, h->f[h->cur], buf, chunk_bytes_of(h), h->stream),
+       "halo copy kernel launch");
+    h->launches++;
+    return UFS_DVM_OK;
+}
+int ufs_dvm_halo_pack(ufs_dvm_t h, int32_t peer, void* buf_dev) { return halo_copy(h, peer, buf_dev, true); }
+int ufs_dvm_halo_unpack(ufs_dvm_t h, int32_t peer, const void* buf_dev) { return halo_copy(h, peer, const_cast<void*>(buf_dev), false); }
+
+int ufs_dvm_halo_done(ufs_dvm_t h) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    const FlatMesh& m = h->mesh;
+    const int64_t n_gh = m.n_slabs - m.n_kin;
+    if (n_gh > 0 && h->plan.ring >= 2) {
+        // the velocity sums of the ghost cells, from the chunks that have just arrived (the step's Maxwellian needs
+        // the upwind flux moments of every source; entries of chunks that never arrive are never read)
+        StepParams p = make_params(h, 1.0);
+        p.n_kin = (int32_t)n_gh;
+        const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
+        const char* f = static_cast<const char*>(h->f[h->cur]) + (size_t)m.n_kin * m.vel.Nv * elem;
+        CU(launch_sums(h->storage, h->plan, p, f, h->d_sums[h->cur] + (size_t)m.n_kin * SUMS_STRIDE, h->stream), "ghost sums kernel launch");
+        h->launches++;
+    }
+    h->ghosts_fresh = true;
     return UFS_DVM_OK;
 }
 

@@ -405,6 +405,146 @@ int flatten(const ufs_dvm_desc& d, FlatMesh& m, std::string& err) {
         }
         m.octet_start[s] = all ? 1 : 0;
     }
+    m.n_slabs = m.n_kin;
+    return UFS_DVM_OK;
+}
+
+// ---- multi-GPU: N-order partition and one rank's part of the mesh ----------------------------
+int partition_leaves(const ufs_dvm_desc& d, int n_ranks, double w_kinetic, double w_fluid, int32_t* rank_of_leaf, std::string& err) {
+    if (d.n_leaves <= 0 || !d.level || !d.ijk || !d.kind || !rank_of_leaf) { err = "empty or NULL leaf list"; return UFS_DVM_EINVAL; }
+    if (n_ranks < 1) { err = "n_ranks must be at least 1"; return UFS_DVM_EINVAL; }
+    if (!(w_kinetic > 0) || !(w_fluid >= 0)) { err = "weights: w_kinetic > 0, w_fluid >= 0"; return UFS_DVM_EINVAL; }
+    const int64_t n = d.n_leaves;
+    int lmax = 0;
+    for (int64_t j = 0; j < n; j++) {
+        if (d.level[j] > 18) { err = "level > 18"; return UFS_DVM_EINVAL; }
+        lmax = std::max<int>(lmax, d.level[j]);
+    }
+    std::vector<uint64_t> key(n);
+    for (int64_t j = 0; j < n; j++) {
+        const int sh = lmax - d.level[j];
+        const uint32_t* c = d.ijk + 3 * j;
+        key[j] = morton((uint64_t)c[0] << sh, (uint64_t)c[1] << sh, (uint64_t)c[2] << sh);
+    }
+    std::vector<int64_t> order(n);
+    std::iota(order.begin(), order.end(), (int64_t)0);
+    std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return key[a] != key[b] ? key[a] < key[b] : d.level[a] < d.level[b]; });
+    auto weight = [&](int64_t j) { return d.kind[j] == UFS_CELL_KINETIC ? w_kinetic : d.kind[j] == UFS_CELL_FLUID ? w_fluid : 0.0; };
+    long double total = 0;
+    for (int64_t j = 0; j < n; j++) total += weight(j);
+    if (!(total > 0)) { err = "the mesh has no leaf of positive weight"; return UFS_DVM_EINVAL; }
+    long double before = 0;
+    int last = 0;
+    for (int64_t r = 0; r < n; r++) {
+        const int64_t j = order[r];
+        int rk = (int)(before * n_ranks / total);
+        rk = std::min(std::max(rk, last), n_ranks - 1);   // monotone along the curve whatever the rounding does
+        rank_of_leaf[j] = rk;
+        last = rk;
+        before += weight(j);
+    }
+    return UFS_DVM_OK;
+}
+
+int restrict_to_rank(FlatMesh& m, const int32_t* rank_of_leaf, int my_rank, int n_ranks, std::string& err) {
+    if (!rank_of_leaf || n_ranks < 1 || my_rank < 0 || my_rank >= n_ranks) { err = "bad rank arguments"; return UFS_DVM_EINVAL; }
+    const int64_t NG = m.n_kin;   // slabs of the whole mesh
+    // the rank's kinetic leaves must be one range of consecutive slabs (a range of the N-order curve)
+    int64_t g0 = -1, g1 = -1;
+    for (int64_t s = 0; s < NG; s++) {
+        const int32_t rk = rank_of_leaf[m.cell_of_slab[s]];
+        if (rk < 0 || rk >= n_ranks) { err = "rank_of_leaf out of range"; return UFS_DVM_EINVAL; }
+        if (rk != my_rank) continue;
+        if (g0 < 0) g0 = s;
+        else if (g1 != s) { err = "the kinetic leaves of a rank must be consecutive in N-order (Morton) among the kinetic leaves"; return UFS_DVM_EINVAL; }
+        g1 = s + 1;
+    }
+    if (g0 < 0) g0 = g1 = 0;
+    const int64_t n_in = g1 - g0;
+    auto octants_of_dir = [](int dd) -> uint8_t {   // octants whose upwind side on axis dd/2 is side dd%2 (low side: xi > 0)
+        uint8_t mk = 0;
+        for (int o = 0; o < 8; o++)
+            if (((o >> (dd >> 1)) & 1) == 1 - (dd & 1)) mk |= (uint8_t)(1u << o);
+        return mk;
+    };
+    // what each rank needs of the slabs it does not own: need[slab] = octant mask, per needing rank (sparse maps)
+    std::vector<std::vector<std::pair<int64_t, uint8_t>>> wanted_from_me(n_ranks);   // (my global slab, mask) wanted by rank p
+    std::vector<std::pair<int64_t, uint8_t>> my_ghosts;                             // (global slab, mask) I want
+    {
+        std::vector<uint8_t> mine(NG, 0);                       // masks of the ghosts I want
+        std::vector<std::vector<uint8_t>> theirs;               // per peer: masks over MY slabs [g0, g1)
+        theirs.assign(n_ranks, std::vector<uint8_t>());
+        for (int64_t s = 0; s < NG; s++) {
+            const int32_t rk = rank_of_leaf[m.cell_of_slab[s]];
+            const CellRec& r = m.recs[s];
+            for (int dd = 0; dd < 6; dd++)
+                for (int k = 0; k < 4; k++) {
+                    const int32_t code = r.src[dd][k];
+                    if (code < 0 || (code >> SRC_SHIFT) != SRC_SLAB) continue;
+                    const int64_t q = code & SRC_INDEX_MASK;
+                    const int32_t rq = rank_of_leaf[m.cell_of_slab[q]];
+                    if (rq == rk) continue;
+                    if (rk == my_rank) mine[q] |= octants_of_dir(dd);
+                    else if (rq == my_rank) {
+                        if (theirs[rk].empty()) theirs[rk].assign(n_in, 0);
+                        theirs[rk][q - g0] |= octants_of_dir(dd);
+                    }
+                }
+        }
+        for (int64_t q = 0; q < NG; q++)
+            if (mine[q]) my_ghosts.emplace_back(q, mine[q]);
+        for (int pr = 0; pr < n_ranks; pr++)
+            for (int64_t i = 0; i < (int64_t)theirs[pr].size(); i++)
+                if (theirs[pr][i]) wanted_from_me[pr].emplace_back(g0 + i, theirs[pr][i]);
+    }
+    const int64_t n_gh = (int64_t)my_ghosts.size();
+    if (n_in + n_gh >= (1 << SRC_SHIFT)) { err = "too many slabs for the 28-bit source index"; return UFS_DVM_EINVAL; }
+    // local numbering: inner slabs first, ghosts after, both in ascending global order
+    std::vector<int64_t> local_of_global(NG, -1);
+    for (int64_t s = g0; s < g1; s++) local_of_global[s] = s - g0;
+    for (int64_t i = 0; i < n_gh; i++) local_of_global[my_ghosts[i].first] = n_in + i;
+    std::vector<CellRec> recs(m.recs.begin() + g0, m.recs.begin() + g1);
+    for (auto& r : recs)
+        for (int dd = 0; dd < 6; dd++)
+            for (int k = 0; k < 4; k++) {
+                const int32_t code = r.src[dd][k];
+                if (code < 0) continue;
+                const int kind = code >> SRC_SHIFT;
+                if (kind != SRC_SLAB && kind != SRC_MIRROR) continue;
+                r.src[dd][k] = src_code((SrcKind)kind, local_of_global[code & SRC_INDEX_MASK]);
+            }
+    std::vector<int64_t> cell_of_slab(n_in + n_gh);
+    for (int64_t s = 0; s < n_in; s++) cell_of_slab[s] = m.cell_of_slab[g0 + s];
+    m.ghost_owner.assign(n_gh, 0);
+    m.send_slab.assign(n_ranks, {}); m.recv_slab.assign(n_ranks, {});
+    m.send_mask.assign(n_ranks, {}); m.recv_mask.assign(n_ranks, {});
+    for (int64_t i = 0; i < n_gh; i++) {
+        const int64_t leaf = m.cell_of_slab[my_ghosts[i].first];
+        cell_of_slab[n_in + i] = leaf;
+        const int32_t ow = rank_of_leaf[leaf];
+        m.ghost_owner[i] = ow;
+        m.recv_slab[ow].push_back((int32_t)(n_in + i));
+        m.recv_mask[ow].push_back(my_ghosts[i].second);
+    }
+    for (int pr = 0; pr < n_ranks; pr++)
+        for (const auto& e : wanted_from_me[pr]) {
+            m.send_slab[pr].push_back((int32_t)(e.first - g0));
+            m.send_mask[pr].push_back(e.second);
+        }
+    std::vector<uint8_t> octet(n_in, 0);
+    for (int64_t s = 0; s + 7 < n_in; s++) octet[s] = m.octet_start[g0 + s];
+    m.octet_start.swap(octet);
+    m.recs.swap(recs);
+    m.cell_of_slab.swap(cell_of_slab);
+    std::fill(m.slab_of_leaf.begin(), m.slab_of_leaf.end(), (int64_t)-1);
+    for (int64_t s = 0; s < n_in + n_gh; s++) m.slab_of_leaf[m.cell_of_slab[s]] = s;
+    m.n_kin = n_in;
+    m.n_slabs = n_in + n_gh;
+    m.partial = true;
+    m.my_rank = my_rank; m.n_ranks = n_ranks;
+    m.first_global_slab = g0;
+    m.n_simple = 0;
+    for (const auto& r : m.recs) m.n_simple += (r.flags & CELL_SIMPLE) ? 1 : 0;
     return UFS_DVM_OK;
 }
 

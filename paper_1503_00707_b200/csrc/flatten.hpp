@@ -88,6 +88,18 @@ static_assert(sizeof(TileHdr) == 32, "TileHdr must be 32 bytes");
 
 struct FlatMesh {
     int64_t n_leaves = 0, n_kin = 0;
+    // ---- one rank's part of a partitioned mesh (restrict_to_rank).  n_kin counts the rank's own
+    // ("inner") kinetic leaves, stored first; the ghost cells -- kinetic leaves of other ranks that are upwind sources of
+    // inner cells -- follow ("inner cells are stored before ghost cells").  Unpartitioned: n_slabs = n_kin.
+    int64_t n_slabs = 0;
+    bool partial = false;
+    int32_t my_rank = 0, n_ranks = 1;
+    int64_t first_global_slab = 0;             // inner slab s is slab first_global_slab + s of the whole mesh
+    std::vector<int32_t> ghost_owner;          // [n_slabs - n_kin] rank that owns each ghost cell
+    // per peer rank: the chunks to send (inner slab, octant mask) and to receive (ghost slab, octant mask), both in
+    // ascending order of the cell's global slab number, so that the k-th entry sent is the k-th entry the peer expects
+    std::vector<std::vector<int32_t>> send_slab, recv_slab;
+    std::vector<std::vector<uint8_t>> send_mask, recv_mask;
     int lmax = 0;
     std::vector<int64_t> order;         // Morton rank -> leaf
     std::vector<int64_t> rank;          // leaf -> Morton rank
@@ -139,6 +151,16 @@ struct RemapPlan {
     int64_t n_copy = 0, n_prolong = 0, n_restrict = 0, n_from_fluid = 0;
 };
 int build_remap(const FlatMesh& old_mesh, const FlatMesh& new_mesh, RemapPlan& plan, std::string& err);
+
+// Space-filling-curve partition (Fig. 3): the leaves in N-order, each weighted by its cost (w_kinetic for
+// KINETIC, w_fluid for FLUID, 0 for SOLID), cut into n_ranks consecutive ranges of equal weight: leaf number r of the
+// curve goes to rank floor(W_before(r) * n_ranks / W_total), so every rank's weight is within one leaf of the mean.
+int partition_leaves(const ufs_dvm_desc& d, int n_ranks, double w_kinetic, double w_fluid, int32_t* rank_of_leaf, std::string& err);
+
+// Turns the flattened WHOLE mesh into rank `my_rank`'s part: the rank's kinetic leaves (one range of consecutive slabs)
+// first, then its ghost cells; gather records renumbered; the halo lists of every peer.  Face lists, ghost-state tables
+// and the leaf arrays stay those of the whole mesh.
+int restrict_to_rank(FlatMesh& m, const int32_t* rank_of_leaf, int my_rank, int n_ranks, std::string& err);
 
 // Groups the slabs into tiles whose piece lists hold at most `pmax` pieces per octant (complete sibling octets where
 // the mesh has them, else runs of consecutive slabs) and fills the tile arrays of `m`.

@@ -93,6 +93,9 @@ cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepPara
 cudaError_t launch_remap(int storage, const void* f_old, void* f_new, const int64_t* off, const int32_t* src, const double* wgt,
                          const FluidGhost* ghosts, const uchar4* slot_k, int64_t n_new, int64_t Nv, int sm_count, cudaStream_t stream);
 
+// halo.cu: ghost-cell exchange of a partitioned mesh: chunk list -> contiguous buffer (pack) or back (unpack)
+cudaError_t launch_halo_copy(bool pack, const int32_t* chunks, int64_t n_chunks, void* f, void* buf, int64_t chunk_bytes, cudaStream_t stream);
+
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 
