@@ -89,7 +89,11 @@ int ufs_dvm_create_host(const ufs_dvm_desc *desc, ufs_dvm_t *out);
  * (k_tiles where the velocity grid has 12 positive nodes on x and whole 48-row blocks, e.g. 24^3; else k_rows,
  * k_stream, or the one-CTA-per-cell kernels, which need no k_prep); one more pass (the velocity sums of f) before
  * the first step and after ufs_dvm_f_changed.  The environment variable UFS_DVM_KERNEL = rows | stream | cell (read at
- * creation) forces the later kernels of that list (A/B timing, tests of the fallbacks). */
+ * creation) forces the later kernels of that list (A/B timing, tests of the fallbacks).
+ * Every wait inside the persistent kernels has a wall-clock watchdog (2 s without progress): a protocol bug or a faulted
+ * copy ends the kernel with a trap, reported as UFS_DVM_ECUDA by ufs_dvm_sync (the CUDA context is then lost, as after
+ * any device fault), never a hung GPU.  UFS_DVM_TEST_STALL (read at creation) makes k_tiles withhold one barrier arrival on
+ * purpose so that tests can see exactly that. */
 int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps);
 
 /* Enqueue the moments of the current f: mom_dev is DEVICE memory, [5][n_kinetic] doubles in slab order:

@@ -191,6 +191,7 @@ int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out, const int32_t* rank_
         } else if (!want_vec && rows_plan(h->storage, h->mesh.vel, 1, &cand)) h->plan = cand;
         else if (stream_plan(h->storage, h->mesh.vel, 1, &cand)) h->plan = cand;
     }
+    h->plan.test_stall = std::getenv("UFS_DVM_TEST_STALL") ? 1 : 0;
     return UFS_DVM_OK;
 }
 

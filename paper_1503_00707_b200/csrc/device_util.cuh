@@ -7,8 +7,10 @@
 
 namespace ufs {
 
-#ifndef UFS_WAIT_SPINS
-#define UFS_WAIT_SPINS 512u   // watchdog of smbar_wait (x 10 ms suspend hint); the test of the trap path builds with 2
+// Watchdog of the persistent kernels' waits: a wait that lasts this long (wall clock, %globaltimer) can only be a
+// protocol bug or a faulted copy.
+#ifndef UFS_WAIT_TIMEOUT_NS
+#define UFS_WAIT_TIMEOUT_NS 2000000000ull
 #endif
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -94,14 +96,19 @@ __device__ __forceinline__ bool smbar_try_wait(uint32_t bar, uint32_t parity) {
                  : "=r"(ok) : "r"(bar), "r"(parity), "r"(0x989680u) : "memory");
     return ok != 0;
 }
-// Waits of the persistent kernels.  Every try_wait suspends for up to the hint above (10 ms); 512 of them without the
-// phase completing (seconds) can only be a protocol bug or a faulted copy: trap, so that the failure surfaces as
-// UFS_DVM_ECUDA at ufs_dvm_sync instead of hanging the GPU.  The counter lives in the slow path only.
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t;
+}
+// Waits of the persistent kernels.  try_wait suspends the thread in hardware until the phase completes or a short,
+// hardware-defined time has passed (the hint above is an upper bound, in practice a fraction of a microsecond), so the
+// loop is not a busy spin.  The watchdog is a wall-clock one: UFS_WAIT_TIMEOUT_NS without the phase completing traps, so
+// that the failure surfaces as UFS_DVM_ECUDA at ufs_dvm_sync instead of hanging the GPU; a kernel slowed down many times
+// over (a profiler's replay pass, a debugger) does not trip it.  The timer is read in the slow path only.
 __device__ __forceinline__ void smbar_wait(uint32_t bar, uint32_t parity) {
     if (smbar_try_wait(bar, parity)) return;
-    uint32_t spins = 0;
+    const unsigned long long t0 = globaltimer_ns();
     while (!smbar_try_wait(bar, parity)) {
-        if (++spins > UFS_WAIT_SPINS) __trap();
+        if (globaltimer_ns() - t0 > UFS_WAIT_TIMEOUT_NS) __trap();
     }
 }
 __device__ __forceinline__ void sbulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {

@@ -60,6 +60,7 @@ struct StepLaunch {
                                    // 2: streaming step, one vector per thread (step_stream.cu), 0: one CTA per cell (kernels.cu)
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
     cudaEvent_t ev0, ev1;          // if set: recorded on the stream right before / after the main kernel of the step
+    int32_t test_stall;            // UFS_DVM_TEST_STALL was set at creation: k_tiles stalls on purpose (watchdog test)
 };
 
 // per-axis table stride (nodes rounded up to a multiple of 4)

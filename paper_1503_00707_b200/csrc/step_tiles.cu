@@ -224,7 +224,9 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     const uint32_t fb = sb + o_full + 8u * slot;
                     const uint32_t dsc = sb + o_desc + slot * DESC_BYTES;
                     const int mine = npk > w ? (npk + 3 - w) >> 2 : 0;   // pieces this warp copies
-                    if (lane == 0) {
+                    // (test hook, UFS_DVM_TEST_STALL: one producer warp withholds its arrival on the fourth stage; the
+                    // consumers' wait then runs into the watchdog, include/ufs_dvm.h)
+                    if (lane == 0 && !(p.smap[11] && k == 3 && w == 1)) {
                         if (w == 0) ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
                         const uint32_t extra = (w == 0 && !SUMS_ONLY) ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u;
                         smbar_arrive_expect_tx(fb, (uint32_t)mine * PB + extra);
@@ -536,6 +538,7 @@ cudaError_t launch_tiles_t(const StepLaunch& plan, const StepParams& p, cudaStre
     const TilesSmem m = tiles_map(sizeof(T), plan.stages, tabn_of(p.nh));
     const uint32_t v[11] = {m.ring, m.desc, m.thdr, m.red, m.full, m.empty, m.tinfo, m.ttab, m.tempty, m.total, m.thdr_bytes};
     for (int i = 0; i < 11; i++) q.smap[i] = v[i];
+    q.smap[11] = plan.test_stall ? 1u : 0u;
     q.ring_stages = plan.stages;
     if (timed && plan.ev0) cudaEventRecord(plan.ev0, st);
     kfn<<<grid, (N_PROD + N_CONS) * 32, plan.smem_bytes, st>>>(q);

@@ -190,3 +190,38 @@ def test_uniform_maxwellian_steady_on_gpu():
     st.sync()
     assert rel_linf(st.read_canonical(), f0) < 5e-14
     st.close()
+
+
+def test_stalled_pipeline_traps_and_is_reported_not_hung():
+    """Every wait of the persistent kernel has a wall-clock watchdog (device_util.cuh: smbar_wait): with the test hook
+    UFS_DVM_TEST_STALL one producer warp withholds a barrier arrival, the consumers' wait times out, the kernel traps and
+    ufs_dvm_sync returns UFS_DVM_ECUDA.  Run in a child process: a device trap takes the CUDA context with it."""
+    import os
+    import subprocess
+    import sys
+    import time
+    code = (
+        "import sys, time\n"
+        "from paper_1503_00707_b200 import binding as B, inputs\n"
+        "case = inputs.small(3)\n"
+        "st = B.DvmStepper(case)\n"
+        "assert B.ufs_dvm_kernel_name(st.h) == 'k_tiles'\n"
+        "st.load_canonical(inputs.initial_f(case))\n"
+        "t0 = time.time()\n"
+        "try:\n"
+        "    st.step(case.dt, 1)\n"
+        "    st.sync()\n"
+        "    print('NO ERROR')\n"
+        "except B.UfsDvmError as e:\n"
+        "    print('CODE', e.code, 'SECONDS %.1f' % (time.time() - t0))\n"
+        "sys.stdout.flush()\n"
+        "import os; os._exit(0)\n")
+    env = dict(os.environ, UFS_DVM_TEST_STALL="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    t0 = time.time()
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=120)
+    assert f"CODE {B.ECUDA}" in res.stdout, res.stdout + res.stderr
+    assert time.time() - t0 < 60            # seconds, not a hang
+    # and the same process without the hook is fine
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ), capture_output=True, text=True, timeout=120)
+    assert "NO ERROR" in res.stdout, res.stdout + res.stderr
