@@ -8,8 +8,10 @@ SURVEY.md 8(d) row 4); both f buffers (2 x 55.8 GB) resident in HBM.  Synthetic,
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3|config5]
     python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
+    python bench.py --emulate-ranks R ...     # 1 GPU: the workload cut into R ranks with the ghost exchange
+    torchrun ... bench.py --gpus N --partition  # one partitioned problem over N GPUs (NCCL ghost exchange)
 
-N > 1 runs N independent replicas (the path is one GPU by the north star).
+N > 1 runs N independent replicas by default (the path is one GPU by the north star).
 """
 import argparse
 import json
@@ -52,19 +54,19 @@ def peaks():
 
 
 def ncu_traffic_ratio(workload: str):
-    """DRAM bytes per algorithmic byte of the step kernel from the committed ncu capture, or None."""
+    """DRAM bytes per algorithmic byte of the step kernel from the committed ncu capture of exactly this workload
+    (profiles/step_kernel_traffic.csv), or None if there is no such row."""
     path = os.path.join(ROOT, "profiles", "step_kernel_traffic.csv")
     if not os.path.exists(path):
         return None
-    best = None
     with open(path) as fh:
         for line in fh:
             if line.startswith("#") or not line.strip():
                 continue
             w, storage, alg, rd, wr = line.strip().split(",")[:5]
-            if w.startswith(workload.split("_")[0]):
-                best = (float(rd) + float(wr)) / float(alg)
-    return best
+            if w == workload:
+                return (float(rd) + float(wr)) / float(alg)
+    return None
 
 
 def oracle_sample(case, n_sample: int):
@@ -146,6 +148,97 @@ def aggregate_over_ranks(ms_local: float, units_local: float, device=None):
     return float(t.item()), float(u.item())
 
 
+def run_partitioned(args):
+    """The partitioned step (include/ufs_dvm.h "Partitioned mesh"): the workload cut along the
+    N-order curve into equal-weight ranks, ghost chunks exchanged before every step.  Under torchrun every process is
+    one rank (NCCL send / recv, strong scaling of ONE problem); with --emulate-ranks R the R ranks live on one GPU and
+    one stream and the transfer is a device copy, which measures what the exchange costs besides the wire."""
+    import torch
+    import torch.distributed as dist
+    from paper_1503_00707_b200 import binding as B
+    from paper_1503_00707_b200 import harness
+    from paper_1503_00707_b200.partition import RankStepper, exchange_distributed, exchange_local
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the DVM step has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    emulate = args.emulate_ranks if world == 1 else 0
+    n_ranks = emulate if emulate else world
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    case = make_case(args.workload)
+    desc, keep = B.make_desc(case)
+    rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, 0.0)
+    mine = list(range(n_ranks)) if emulate else [rank]
+    ranks = [RankStepper(case, rol, r, n_ranks, device=dev) for r in mine]
+    for st in ranks:
+        harness.fill_initial_f_device(st, case)
+    stream = ranks[0].stream
+
+    def exchange():
+        if emulate:
+            exchange_local(ranks)
+        else:
+            exchange_distributed(ranks[0])
+
+    def step(k):
+        for _ in range(k):
+            exchange()
+            for st in ranks:
+                st.step(case.dt, 1)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    step(args.warmup)
+    barrier()
+    launches0 = sum(B.ufs_dvm_launch_count(st.h) for st in ranks)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    with harness.ClockSampler(index=torch.cuda.current_device()) as clk:
+        ev[0].record(stream)
+        step(args.steps)
+        ev[1].record(stream)
+        barrier()
+    launches = sum(B.ufs_dvm_launch_count(st.h) for st in ranks) - launches0
+    ev[2].record(stream)                       # the exchange alone (pack, transfer, unpack, ghost sums)
+    for _ in range(args.steps):
+        exchange()
+    ev[3].record(stream)
+    barrier()
+    for st in ranks:
+        st.sync()
+    ms, ms_x = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3])
+    n_inner = sum(st.n_inner for st in ranks)
+    ms, units = aggregate_over_ranks(ms, float(n_inner * case.Nv * args.steps), dev)
+    ms_x, _ = aggregate_over_ranks(ms_x, 0.0, dev)
+    sent = sum(st.halo_bytes()[0] for st in ranks)
+    ghosts = sum(st.n_ghost for st in ranks)
+    elem = 4 if case.storage == 1 else 8
+    cfg = workload_config(case, args)
+    cfg["parallelism"] = (f"{n_ranks} ranks emulated on 1 GPU, one stream (device copy instead of NCCL)" if emulate
+                          else f"{n_ranks} ranks, one GPU each, NCCL send/recv of the packed ghost chunks")
+    line = {"metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
+            "dtype": "f32" if case.storage == 1 else "f64", "data": "synthetic", "config": cfg, "clocks": clk.summary(),
+            "e2e": None, "gpu_launches": launches,
+            "halo": {"ranks": n_ranks, "inner_cells_this_process": n_inner, "ghost_cells_this_process": ghosts,
+                     "ghost_fraction": ghosts / max(n_inner, 1), "sent_bytes_per_step_this_process": sent,
+                     "sent_fraction_of_f": sent / max(n_inner * case.Nv * elem, 1),
+                     "exchange_ms_per_step": ms_x / args.steps, "exchange_share_of_step": ms_x / ms}}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    for st in ranks:
+        st.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def workload_config(case, args):
     return {"workload": f"{args.workload}: {case.name}, {int((case.kind == 0).sum())} kinetic leaves "
                         f"(levels {int(case.level.min())}-{int(case.level.max())}), velocity grid "
@@ -164,11 +257,17 @@ def main():
     ap.add_argument("--workload", default="config4")
     ap.add_argument("--oracle-leaves", type=int, default=0, help="size of the CPU-oracle sample (0 = default)")
     ap.add_argument("--kn", type=float, default=None, help="override the Knudsen number (inf = collisions off)")
+    ap.add_argument("--partition", action="store_true",
+                    help="N > 1: one partitioned problem over the ranks (ghost exchange) instead of N replicas")
+    ap.add_argument("--emulate-ranks", type=int, default=0,
+                    help="1 GPU: cut the workload into R ranks on this GPU and step them with the ghost exchange")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.emulate_ranks > 1 or (args.partition and int(os.environ.get("WORLD_SIZE", "1")) > 1):
+        return run_partitioned(args)
 
     import torch
     import torch.distributed as dist
@@ -256,7 +355,7 @@ def main():
     ratio = ncu_traffic_ratio(args.workload)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None if ratio is None else ratio * alg_bytes_per_launch,
-                "traffic_source": None if ratio is None else "profiles/step_kernel_traffic.csv: ncu dram bytes per algorithmic byte x this launch's algorithmic bytes",
+                "traffic_source": None if ratio is None else f"profiles/step_kernel_traffic.csv row '{args.workload}': ncu dram bytes per algorithmic byte x this launch's algorithmic bytes",
                 "peak_source": peak_src, "kernel": kernel_name, "kernel_ms": kernel_ms, "kernel_launches_timed": kernel_n,
                 "kernel_share_of_step": kernel_ms / (ms_local / args.steps),
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch,

@@ -29,14 +29,15 @@ def fill_initial_f_device(st: "B.DvmStepper", case: Case, chunk_slabs: int = 204
     prim = torch.as_tensor(case.prim0[st.cell_of_slab], device=dev)            # [n_kin, 5] in slab order
     with torch.cuda.stream(st.stream):           # ordered with the handle's stream
         for s0 in range(0, st.n_kinetic, chunk_slabs):
-            p = prim[s0:s0 + chunk_slabs]
+            s1 = min(s0 + chunk_slabs, st.n_kinetic)     # (a partitioned handle's tensors hold ghost slabs after these)
+            p = prim[s0:s1]
             n, ux, uy, uz, T = (p[:, c:c + 1] for c in range(5))
             ex = torch.exp(-(xs[None, :] - ux) ** 2 / (2 * T))
             ey = torch.exp(-(ys[None, :] - uy) ** 2 / (2 * T))
             ez = torch.exp(-(zs[None, :] - uz) ** 2 / (2 * T))
             a = n / (2 * np.pi * T) ** 1.5
             f = a * ez[:, kz] * ey[:, ky] * ex[:, kx]
-            st.f[cur][s0:s0 + chunk_slabs].copy_(f.to(st.dtype))
+            st.f[cur][s0:s1].copy_(f.to(st.dtype))
     B.ufs_dvm_f_changed(st.h)
 
 
