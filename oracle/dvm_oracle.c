@@ -258,6 +258,15 @@ int oracle_dvm_create(const oracle_desc *d, oracle_t **out) {
 }
 
 int64_t oracle_dvm_n_kinetic(const oracle_t *o) { return o->n_kin; }
+/* Replaces the ghost state of INFLOW side `side` by a caller-given table values[Nv] (canonical velocity order).  The
+ * lattice-Boltzmann variant (oracle/lbm_oracle.py) puts its polynomial equilibrium there (the weights serve
+ * "the equilibrium distribution function for initial and boundary conditions"); the arithmetic of S2/S3 is unchanged. */
+int oracle_dvm_set_inflow_table(oracle_t *o, int side, const double *values) {
+    if (!o || side < 0 || side >= 6 || !values) return -1;
+    memcpy(o->inflow_f + (size_t)side * o->Nv, values, (size_t)o->Nv * sizeof(double));
+    return 0;
+}
+
 void oracle_dvm_kinetic_leaves(const oracle_t *o, int64_t *leaf_of_row) { memcpy(leaf_of_row, o->kin_leaf, o->n_kin * 8); }
 
 /* ---- S2 + S3 for one kinetic leaf: fstar[Nv] from f (all kinetic rows) ---- */

@@ -40,6 +40,7 @@ def lib():
         L.oracle_dvm_kinetic_leaves.argtypes = [C.c_void_p, C.c_void_p]
         L.oracle_dvm_remap.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.oracle_dvm_set_threads.argtypes = [C.c_int]
+        L.oracle_dvm_set_inflow_table.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         _lib = L
     return _lib
 
@@ -92,6 +93,13 @@ class Oracle:
         if rc != 0:
             raise OracleError(rc, "Newton failed" if rc == -5 else "")
         return out
+
+    def set_inflow_table(self, side, values):
+        """Ghost state of INFLOW side `side` given as a table [Nv] (canonical velocity order) instead of a Maxwellian."""
+        v = np.ascontiguousarray(values, np.float64)
+        assert v.shape == (self.Nv,)
+        rc = lib().oracle_dvm_set_inflow_table(self._h, int(side), v.ctypes.data)
+        assert rc == 0
 
     def transport(self, f, dt):
         return self._run(lib().oracle_dvm_transport, f, dt)

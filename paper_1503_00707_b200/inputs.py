@@ -439,3 +439,51 @@ def with_body_of(old: Case, new: Case, name: Optional[str] = None) -> Case:
         out.kind[idx] = CELL_SOLID
     out.name = name or (new.name + "_body_of_" + old.name)
     return out
+
+
+# ----------------------------------------------------------------------------------------------
+# lattice-Boltzmann variant: problem statements only.  The lattice itself (velocities, weights) is
+# textbook data both sides need to agree on what an index means; the equilibrium formula is NOT here (each side has its own).
+# ----------------------------------------------------------------------------------------------
+def lattice_velocities(q: int) -> np.ndarray:
+    """c_i [Q,3] in {-1,0,1}^3 for D3Q27 (all 27) or D3Q19 (|c|^2 <= 2), in ascending canonical index
+    (kz*3 + ky)*3 + kx with c = k - 1 -- the 3x3x3 velocity grid of the DVM solver."""
+    assert q in (19, 27)
+    k = np.arange(27)
+    c = np.stack([k % 3 - 1, (k // 3) % 3 - 1, k // 9 - 1], axis=1)
+    keep = (c ** 2).sum(axis=1) <= (2 if q == 19 else 3)
+    return c[keep].astype(np.int64)
+
+
+def lbm_case(tree: Case, lattice: int = 19, omega: float = 0.7, cfl: float = 0.4, nsteps: int = 5, mach: float = 0.1,
+             storage: int = STORE_F64, noise_rel: float = 1e-3, seed: int = 0) -> Case:
+    """An LBM problem on the mesh, boundary codes and solid leaves of `tree`: 3x3x3 velocity grid on [-1.5,1.5]^3 (nodes
+    -1, 0, 1: lattice units, c_s^2 = 1/3), D3Q19 or D3Q27, relaxation time tau = dt / omega, initial state
+    rho = 1 + 0.05 sin(2 pi x) cos(2 pi y), u = Ma c_s (cos 2 pi z, 0.5 sin 2 pi x, -0.3) (smooth, all components alive);
+    INFLOW sides carry (rho, u) = (1, Ma c_s e_x).  FLUID leaves of the tree become KINETIC (the LBM has no mask)."""
+    import copy
+    c = copy.copy(tree)
+    c.name = f"lbm_d3q{lattice}_{tree.name}"
+    c.kind = np.where(tree.kind == CELL_SOLID, CELL_SOLID, CELL_KINETIC).astype(np.uint8)
+    c.fluid_moments = None
+    c.nv, c.vmin, c.vmax = (3, 3, 3), (-1.5,) * 3, (1.5,) * 3
+    c.kn = float("inf")
+    c.storage, c.cfl, c.nsteps = storage, cfl, nsteps
+    x = c.centres()
+    cs = 1.0 / np.sqrt(3.0)
+    prim = np.zeros((c.n_leaves, 5))
+    prim[:, 0] = 1 + 0.05 * np.sin(2 * np.pi * x[:, 0]) * np.cos(2 * np.pi * x[:, 1])
+    prim[:, 1] = mach * cs * np.cos(2 * np.pi * x[:, 2])
+    prim[:, 2] = 0.5 * mach * cs * np.sin(2 * np.pi * x[:, 0])
+    prim[:, 3] = -0.3 * mach * cs
+    prim[:, 4] = 1.0 / 3.0
+    c.prim0 = prim
+    c.inflow = np.zeros((6, 5)); c.inflow[:, 0] = 1.0; c.inflow[:, 1] = mach * cs; c.inflow[:, 4] = 1.0 / 3.0
+    c.noise_rel, c.noise_seed = noise_rel, seed
+    c.meta = dict(tree.meta, lattice=lattice, omega=omega)
+    return c
+
+
+def lbm_tau(case: Case) -> float:
+    """Relaxation time of an lbm_case: dt / omega."""
+    return case.dt / case.meta["omega"]
