@@ -6,7 +6,7 @@ Workload (N=1): the configuration the north-star target is stated on -- the ~1.0
 octree with a 24^3 velocity grid, fp32 storage, fp64 moment accumulation (BASELINE.json configs[3],
 SURVEY.md 8(d) row 4); both f buffers (2 x 55.8 GB) resident in HBM.  Synthetic, seeded inputs.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3|config5]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config4_lit|config4_small|config2|config3|config5|lbm19|lbm27|lbm19_f32|lbm19_small]
     python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
     python bench.py --emulate-ranks R ...     # 1 GPU: the workload cut into R ranks with the ghost exchange
     torchrun ... bench.py --gpus N --partition  # one partitioned problem over N GPUs (NCCL ghost exchange)
@@ -239,6 +239,67 @@ def run_partitioned(args):
         dist.destroy_process_group()
 
 
+def run_lbm(args):
+    """The lattice-Boltzmann variant (include/ufs_lbm.h; Table 1: ~1M cells): D3Q19 / D3Q27 on the
+    config-4 octree (1 009 261 leaves, periodic), one kernel per step.  A "phase-space cell" is (leaf, lattice velocity);
+    algorithmic bytes = one read and one write of f = 2 * Q * sizeof(storage) per leaf."""
+    import torch
+    from paper_1503_00707_b200 import harness, inputs
+    from paper_1503_00707_b200 import lbm as K
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the LBM step has no CPU fallback")
+    q = 27 if "27" in args.workload else 19
+    tree = inputs.config4(base=5, lmax=7, target_leaves=125_000, side_scale=2.0) if args.workload.endswith("_small") else inputs.config4()
+    case = inputs.lbm_case(tree, q, storage=inputs.STORE_F32 if "f32" in args.workload else inputs.STORE_F64)
+    dev = torch.device("cuda", 0)
+    st = K.LbmStepper(case, device=dev)
+    # f(t=0): every cell at rest with its density, w_i rho (weights from the library's layout call)
+    rho = torch.as_tensor(case.prim0[st.cell_of_row, 0], device=dev)
+    st.f[K.ufs_lbm_current(st.h)].copy_((torch.as_tensor(st.w, device=dev)[:, None] * rho[None, :]).to(st.dtype))   # [Q, n]
+    n, elem, dt = st.n_cells, (4 if st.storage == 1 else 8), case.dt
+    st.step(dt, args.warmup)
+    torch.cuda.synchronize(dev)
+    l0 = K.ufs_lbm_launch_count(st.h)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with harness.ClockSampler(index=0) as clk:
+        ev0.record(st.stream)
+        st.step(dt, args.steps)
+        ev1.record(st.stream)
+        torch.cuda.synchronize(dev)
+    st.sync()
+    ms = ev0.elapsed_time(ev1)
+    launches = K.ufs_lbm_launch_count(st.h) - l0
+    peak, peak_src = peaks()
+    alg = 2.0 * n * q * elem
+    rec_bytes = 32.0 * n
+    achieved = alg / (ms * 1e-3 / args.steps) / 1e9
+    line = {"metric": METRIC, "value": n * q * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: D3Q{q} on the config-4 octree, {n} cells (levels {int(case.level.min())}-{int(case.level.max())}), "
+                                   f"omega = dt/tau = {case.meta['omega']}, CFL {case.cfl}",
+                       "storage": "fp32" if st.storage == 1 else "fp64",
+                       "l2": "f buffers (2 x %.0f MB) exceed L2 for the full-size tree" % (n * q * elem / 1e6), "parallelism": "1 GPU"},
+            "clocks": clk.summary(), "e2e": None, "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "peak_source": peak_src, "kernel": "k_lbm_step", "kernel_ms": ms / args.steps,
+                         "algorithmic_bytes_per_launch": alg, "cell_record_bytes_per_launch": rec_bytes,
+                         "frac_with_cell_records": (alg + rec_bytes) / (ms * 1e-3 / args.steps) / 1e9 / peak}}
+    st.close()
+    if not args.no_cpu_baseline:
+        from oracle import dvm_oracle, lbm_oracle
+        sub = oracle_sample(case, args.oracle_leaves or 32768)
+        sub.meta = case.meta
+        o = lbm_oracle.LbmOracle(sub, inputs.lbm_tau(case), window=True)
+        f = lbm_oracle.initial_f(sub)
+        t0 = time.perf_counter()
+        f = o.step(f, dt, 3)
+        t = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": o.n * q * 3 / t, "unit": UNIT, "cores": dvm_oracle.threads(), "kind": "oracle",
+                                "sample": f"first {o.n} Morton-ordered cells, 3 steps (C transport over cells + numpy collision)"}
+    print(json.dumps(line), flush=True)
+
+
 def workload_config(case, args):
     return {"workload": f"{args.workload}: {case.name}, {int((case.kind == 0).sum())} kinetic leaves "
                         f"(levels {int(case.level.min())}-{int(case.level.max())}), velocity grid "
@@ -266,6 +327,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload.startswith("lbm"):
+        return run_lbm(args)
     if args.emulate_ranks > 1 or (args.partition and int(os.environ.get("WORLD_SIZE", "1")) > 1):
         return run_partitioned(args)
 

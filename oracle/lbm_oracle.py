@@ -77,12 +77,12 @@ def moments(q, f):
 class LbmOracle:
     """case: a Case made by inputs.lbm_case (3x3x3 grid on [-1.5,1.5]^3, meta['lattice'], meta['omega'])."""
 
-    def __init__(self, case, tau):
+    def __init__(self, case, tau, window=False):
         assert tuple(case.nv) == (3, 3, 3) and tuple(case.vmin) == (-1.5,) * 3 and tuple(case.vmax) == (1.5,) * 3
         self.q = int(case.meta["lattice"])
         self.tau = float(tau)
         self.c, self.w, self.active = lattice(self.q)
-        self.dvm = Oracle(case, kn=float("inf"))               # L2: transport only
+        self.dvm = Oracle(case, kn=float("inf"), window=window)   # L2: transport only (window: a part of a mesh, bench sample)
         self.n = self.dvm.n_kinetic
         for s in range(6):
             if case.bc[s] == 2:                                 # INFLOW: equilibrium of the side's (rho, u)

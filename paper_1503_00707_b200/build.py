@@ -5,8 +5,9 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libufs_dvm.so")
-SOURCES = ["api.cu", "kernels.cu", "step_stream.cu", "step_rows.cu", "step_tiles.cu", "remap.cu", "halo.cu", "flatten.cpp"]
-HEADERS = ["flatten.hpp", "kernels.cuh", "device_util.cuh", "stream_common.cuh", os.path.join("..", "..", "include", "ufs_dvm.h")]
+SOURCES = ["api.cu", "kernels.cu", "step_stream.cu", "step_rows.cu", "step_tiles.cu", "remap.cu", "halo.cu", "lbm.cu", "flatten.cpp"]
+HEADERS = ["flatten.hpp", "kernels.cuh", "device_util.cuh", "stream_common.cuh", os.path.join("..", "..", "include", "ufs_dvm.h"),
+           os.path.join("..", "..", "include", "ufs_lbm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp,-O3", "--shared", "-lgomp"]
 
