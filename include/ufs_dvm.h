@@ -113,7 +113,11 @@ int ufs_dvm_current(ufs_dvm_t h);
  * per cell, 35 velocity sums of the current f (the moments of Eq. 2's upwind fluxes, that the next
  * step's Maxwellian needs) from one step to the next; after this call they are recomputed from f by one extra
  * pass at the next ufs_dvm_step / ufs_dvm_moments.  Not needed after ufs_dvm_create (nothing is cached yet) nor
- * with ufs_dvm_run_host (it does this itself).  Host-side flag only; returns UFS_DVM_OK. */
+ * with ufs_dvm_run_host (it does this itself).  Host-side flag only; returns UFS_DVM_OK.
+ * A caller that rewrites f and forgets this call gets Maxwellians from stale sums.  Check mode guards against it: with the
+ * environment variable UFS_DVM_CHECK set at creation, every ufs_dvm_step call first re-sums eight pseudo-random cells of
+ * the current f on the device and compares them with the carried sums; a mismatch makes the next ufs_dvm_sync return
+ * UFS_DVM_EINVAL (sixteen small launches per call: for debugging, not for timing). */
 int ufs_dvm_f_changed(ufs_dvm_t h);
 
 /* Layout of the f buffers (HOST outputs, any may be NULL): *n_kinetic; cell_of_slab[n_kinetic] = index into

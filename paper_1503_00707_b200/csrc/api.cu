@@ -41,6 +41,9 @@ struct ufs_dvm_s {
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
+    bool check = false;            // UFS_DVM_CHECK: every step call verifies the carried sums of a few cells against f
+    double* d_check = nullptr;     // scratch of the check
+    uint64_t check_rng = 0x9E3779B97F4A7C15ull;
     bool ghosts_fresh = false;     // the ghost slabs of f[cur] and their sums are those of the peers' current f
     bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
@@ -192,6 +195,7 @@ int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out, const int32_t* rank_
         else if (stream_plan(h->storage, h->mesh.vel, 1, &cand)) h->plan = cand;
     }
     h->plan.test_stall = std::getenv("UFS_DVM_TEST_STALL") ? 1 : 0;
+    h->check = std::getenv("UFS_DVM_CHECK") != nullptr;
     return UFS_DVM_OK;
 }
 
@@ -353,6 +357,18 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
     if (has_ghosts && nsteps == 1 && !h->ghosts_fresh)
         return fail(h, UFS_DVM_EINVAL, "ghost cells are stale: exchange them (ufs_dvm_halo_pack / unpack) and call ufs_dvm_halo_done before the step");
     const bool stream = h->plan.ring >= 2 && h->mesh.n_kin > 0;
+    if (h->check && stream && h->sums_valid && nsteps > 0) {
+        // check mode: the carried sums must still describe f (a caller that rewrote f and forgot ufs_dvm_f_changed gets
+        // UFS_DVM_EINVAL at the next ufs_dvm_sync instead of Maxwellians from stale sums)
+        if (!h->d_check) CU(cudaMalloc(reinterpret_cast<void**>(&h->d_check), SUMS_STRIDE * sizeof(double)), "allocate check scratch");
+        const StepParams p = make_params(h, dt);
+        for (int i = 0; i < 8; i++) {
+            h->check_rng = h->check_rng * 6364136223846793005ull + 1442695040888963407ull;
+            const int64_t cell = (int64_t)((h->check_rng >> 33) % (uint64_t)h->mesh.n_kin);
+            CU(launch_check_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], cell, h->d_check, h->d_flags, h->stream), "check kernel launch");
+            h->launches += 2;
+        }
+    }
     for (int s = 0; s < nsteps; s++) {
         if (stream && !h->sums_valid) {
             const int rc = enqueue_sums(h, make_params(h, dt));
@@ -404,6 +420,10 @@ int ufs_dvm_sync(ufs_dvm_t h) {
     CU(cudaStreamSynchronize(h->stream), "stream synchronize");
     int32_t flags = 0;
     CU(cudaMemcpy(&flags, h->d_flags, 4, cudaMemcpyDeviceToHost), "read flags");
+    if ((flags & 2) && h->sticky == UFS_DVM_OK) {
+        h->sticky = UFS_DVM_EINVAL;
+        h->err = "UFS_DVM_CHECK: the carried velocity sums no longer describe f: f was rewritten without ufs_dvm_f_changed";
+    }
     if ((flags & 1) && h->sticky == UFS_DVM_OK) {
         h->sticky = UFS_DVM_ENEWTON;
         h->err = "Newton iteration for the discrete Maxwellian failed in at least one cell (n <= 0, T <= 0 or no convergence)";
@@ -420,6 +440,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
         cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_tile_fluid);
+        cudaFree(h->d_check);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);

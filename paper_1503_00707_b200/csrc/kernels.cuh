@@ -84,6 +84,9 @@ bool rows_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan);
 cudaError_t launch_rows(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 cudaError_t launch_moments_from_sums(const StepParams& p, const double* sums, double* mom, cudaStream_t stream);
+// check mode: re-sum one cell of f and compare with its carried sums (flags bit 1 on mismatch)
+cudaError_t launch_check_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, const double* carried, int64_t cell,
+                              double* scratch, int32_t* flags, cudaStream_t stream);
 
 // step_tiles.cu: the same step over tiles of up to eight consecutive slabs (shared upwind chunks on chip)
 bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax);

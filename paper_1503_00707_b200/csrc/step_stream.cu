@@ -798,6 +798,25 @@ cudaError_t launch_sums(int storage, const StepLaunch& plan, const StepParams& p
     return cudaGetLastError();
 }
 
+// UFS_DVM_CHECK: flags bit 1 if the freshly formed sums of cell `cell` (in `fresh`) differ from the carried ones
+__global__ void k_check_sums(const double* __restrict__ carried, const double* __restrict__ fresh, int64_t cell, int32_t* flags) {
+    const int j = threadIdx.x;
+    if (j >= 35) return;
+    const double a = carried[cell * SUMS_STRIDE + j], b = fresh[j];
+    const double scale = fabs(carried[cell * SUMS_STRIDE]) + fabs(fresh[0]);   // the cell's density sum
+    if (!(fabs(a - b) <= 1e-6 * scale)) atomicOr(flags, 2);
+}
+cudaError_t launch_check_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, const double* carried, int64_t cell,
+                              double* scratch, int32_t* flags, cudaStream_t st) {
+    StepParams q = p;
+    q.n_kin = 1;
+    const size_t elem = storage == UFS_STORE_F32 ? 4 : 8;
+    cudaError_t e = launch_sums(storage, plan, q, static_cast<const char*>(f) + (size_t)cell * p.Nv * elem, scratch, st);
+    if (e != cudaSuccess) return e;
+    k_check_sums<<<1, 64, 0, st>>>(carried, scratch, cell, flags);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_moments_from_sums(const StepParams& p, const double* sums, double* mom, cudaStream_t st) {
     if (p.n_kin == 0) return cudaSuccess;
     const int64_t n = (int64_t)p.n_kin * 5;

@@ -225,3 +225,27 @@ def test_stalled_pipeline_traps_and_is_reported_not_hung():
     # and the same process without the hook is fine
     res = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ), capture_output=True, text=True, timeout=120)
     assert "NO ERROR" in res.stdout, res.stdout + res.stderr
+
+
+def test_check_mode_catches_a_forgotten_f_changed(monkeypatch):
+    """UFS_DVM_CHECK (include/ufs_dvm.h): rewriting f on the device without ufs_dvm_f_changed is reported as EINVAL at the
+    next sync; with the call, or without a rewrite, nothing is reported."""
+    monkeypatch.setenv("UFS_DVM_CHECK", "1")
+    case = inputs.small(3)
+    f0 = inputs.initial_f(case)
+    st = B.DvmStepper(case)
+    st.load_canonical(f0)
+    st.step(case.dt, 2)
+    st.step(case.dt, 1)
+    st.sync()                                              # clean run: no report
+    cur = B.ufs_dvm_current(st.h)
+    st.f[cur].mul_(1.5)                                    # the caller rewrites f ...
+    B.ufs_dvm_f_changed(st.h)                              # ... and says so
+    st.step(case.dt, 1)
+    st.sync()
+    st.f[B.ufs_dvm_current(st.h)].mul_(1.5)                # ... and forgets to say so
+    st.step(case.dt, 1)
+    with pytest.raises(B.UfsDvmError) as e:
+        st.sync()
+    assert e.value.code == B.EINVAL and "ufs_dvm_f_changed" in str(e.value)
+    st.close()
