@@ -224,14 +224,15 @@ int ufs_dvm_halo_done(ufs_dvm_t h);
 
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
- * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes (bit 31: inflow ghost table, else
- * slab * 8 + octant); cellidx[n_tiles][8][8][16] bytes = per octant and cell: [0] own piece, [1] flags (bit a: axis a
- * has four finer sources, bit 3: a fluid source), [4 + 4a + k] piece of source k on axis a (0xFF unused, 0xFE fluid
- * leaf); fluid[n_tiles][8][24] = fluid ghost of source k of direction d at [d*4+k] (only if the mesh has FLUID
- * leaves); fluid_leaf[*n_fluid_ghosts] = leaf of each fluid ghost.  First-order form of the per-cell, per-sign-group
- * stencil records of PAPER.md:113-115, deduplicated per tile. */
+ * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes: bits 0..29 = index * 8 + octant, the
+ * index being a slab, or an inflow ghost table if bit 31 is set, or a fluid ghost if bit 30 is set (the frozen Maxwellian
+ * of a FLUID leaf: nothing is copied, the kernel's producer warps write the leaf's separable factors into
+ * the slot); cellidx[n_tiles][8][8][16] bytes = per octant and cell: [0] own piece, [1] flags (bit a: axis a has four
+ * finer sources, bit 3: some source is a fluid ghost), [2..3] little-endian mask, bit 4a + k: source k on axis a is a fluid
+ * ghost, [4 + 4a + k] piece of source k on axis a (0xFF unused); fluid_leaf[*n_fluid_ghosts] = leaf of each fluid ghost.
+ * First-order form of the per-cell, per-sign-group stencil records of PAPER.md:113-115, deduplicated per tile. */
 int ufs_dvm_tiles(ufs_dvm_t h, int64_t *n_tiles, int32_t *pmax, int32_t *hdr, uint32_t *pieces, uint8_t *cellidx,
-                  int32_t *fluid, int64_t *n_fluid_ghosts, int64_t *fluid_leaf);
+                  int64_t *n_fluid_ghosts, int64_t *fluid_leaf);
 
 /* Number of kernels this handle has launched so far (step + moments kernels). */
 int64_t ufs_dvm_launch_count(ufs_dvm_t h);

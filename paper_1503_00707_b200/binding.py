@@ -64,7 +64,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_run_host.argtypes = [vp, vp, vp, vp, vp, C.c_double, C.c_int]
         L.ufs_dvm_remesh.argtypes = [vp, C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p), vp]
         L.ufs_dvm_remap_plan.argtypes = [vp, vp, C.POINTER(C.c_int64), vp, vp, vp, C.POINTER(C.c_int64), vp]
-        L.ufs_dvm_tiles.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int32), vp, vp, vp, vp, C.POINTER(C.c_int64), vp]
+        L.ufs_dvm_tiles.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int32), vp, vp, vp, C.POINTER(C.c_int64), vp]
         i32p = C.c_void_p
         L.ufs_dvm_partition.argtypes = [C.POINTER(ufs_dvm_desc), C.c_int32, C.c_double, C.c_double, i32p]
         L.ufs_dvm_create_part.argtypes = [C.POINTER(ufs_dvm_desc), i32p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), vp, C.POINTER(C.c_void_p)]
@@ -293,16 +293,16 @@ def ufs_dvm_halo_done(h):
 def ufs_dvm_tiles(h) -> dict:
     """The flattener's tile records (see include/ufs_dvm.h); empty arrays if the handle uses another kernel."""
     n, pmax, ng = C.c_int64(), C.c_int32(), C.c_int64()
-    _check(h, lib().ufs_dvm_tiles(h, C.byref(n), C.byref(pmax), None, None, None, None, C.byref(ng), None))
+    _check(h, lib().ufs_dvm_tiles(h, C.byref(n), C.byref(pmax), None, None, None, C.byref(ng), None))
     nt, pm = int(n.value), int(pmax.value)
     hdr = np.zeros((nt, 8), np.int32); pieces = np.zeros((nt, 8, max(pm, 1)), np.uint32)
-    cellidx = np.zeros((nt, 8, 8, 16), np.uint8); fluid = np.full((nt, 8, 24), -1, np.int32)
+    cellidx = np.zeros((nt, 8, 8, 16), np.uint8)
     fluid_leaf = np.zeros(int(ng.value), np.int64)
     _check(h, lib().ufs_dvm_tiles(h, C.byref(n), C.byref(pmax), hdr.ctypes.data, pieces.ctypes.data if pm else None,
-                                  cellidx.ctypes.data, fluid.ctypes.data, C.byref(ng), fluid_leaf.ctypes.data))
+                                  cellidx.ctypes.data, C.byref(ng), fluid_leaf.ctypes.data))
     return {"n_tiles": nt, "pmax": pm, "s0": hdr[:, 0].copy(), "nc": hdr[:, 1].copy(),
             "np": hdr[:, 2:4].copy().view(np.uint8).reshape(nt, 8), "level": hdr[:, 4:6].copy().view(np.uint8).reshape(nt, 8),
-            "pieces": pieces, "cellidx": cellidx, "fluid": fluid, "fluid_leaf": fluid_leaf}
+            "pieces": pieces, "cellidx": cellidx, "fluid_leaf": fluid_leaf}
 
 
 def ufs_dvm_run_host(h, f_host_in_ptr: int, f_host_out_ptr: Optional[int], mom_dev_ptr: int, mom_host_ptr: int,

@@ -37,7 +37,6 @@ struct ufs_dvm_s {
     TileHdr* d_tile_hdr = nullptr;
     uint32_t* d_tile_pieces = nullptr;
     uint8_t* d_tile_cellidx = nullptr;
-    int32_t* d_tile_fluid = nullptr;
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
@@ -116,7 +115,7 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.tile_hdr = h->d_tile_hdr;
     p.tile_pieces = h->d_tile_pieces;
     p.tile_cellidx = h->d_tile_cellidx;
-    p.tile_fluid = h->d_tile_fluid;
+    p.tiles_have_fluid = h->mesh.tiles_have_fluid ? 1 : 0;
     p.n_tiles = (int32_t)h->mesh.tiles.size();
     p.tile_pmax = h->mesh.tile_pmax;
     if (v.fast) {
@@ -184,7 +183,9 @@ int create_common(const ufs_dvm_desc* desc, ufs_dvm_t* out, const int32_t* rank_
     if (!want_cell) {
         int pmax = 0;
         StepLaunch cand{};
-        if (!want_vec && !want_rows && tiles_plan(h->storage, h->mesh.vel, 1, &cand, &pmax)) {
+        // (piece codes keep 30 bits for (slab or fluid ghost) * 8 + octant)
+        const bool codes_fit = h->mesh.n_slabs < (int64_t(1) << 27) && (int64_t)h->mesh.fluid.size() < (int64_t(1) << 27);
+        if (!want_vec && !want_rows && codes_fit && tiles_plan(h->storage, h->mesh.vel, 1, &cand, &pmax)) {
             h->plan = cand;
             try {
                 build_tiles(h->mesh, pmax);
@@ -303,7 +304,6 @@ static int create_device(ufs_dvm_t h, void* f_dev[2], void* cuda_stream) {
         if ((rc = upload(h, &h->d_tile_hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr), "upload tile headers"))) return rc;
         if ((rc = upload(h, &h->d_tile_pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4, "upload tile piece lists"))) return rc;
         if ((rc = upload(h, &h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), "upload tile index tables"))) return rc;
-        if ((rc = upload(h, &h->d_tile_fluid, m.tile_fluid.data(), m.tile_fluid.size() * 4, "upload tile fluid ids"))) return rc;
     }
     if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
@@ -439,7 +439,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
-        cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_tile_fluid);
+        cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx);
         cudaFree(h->d_check);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);
@@ -512,7 +512,7 @@ int ufs_dvm_run_host(ufs_dvm_t h, const void* f_host_in, void* f_host_out, doubl
 }
 
 int ufs_dvm_tiles(ufs_dvm_t h, int64_t* n_tiles, int32_t* pmax, int32_t* hdr, uint32_t* pieces, uint8_t* cellidx,
-                  int32_t* fluid, int64_t* n_fluid_ghosts, int64_t* fluid_leaf) {
+                  int64_t* n_fluid_ghosts, int64_t* fluid_leaf) {
     if (!h) return UFS_DVM_EINVAL;
     const FlatMesh& m = h->mesh;
     if (n_tiles) *n_tiles = (int64_t)m.tiles.size();
@@ -520,7 +520,6 @@ int ufs_dvm_tiles(ufs_dvm_t h, int64_t* n_tiles, int32_t* pmax, int32_t* hdr, ui
     if (hdr) std::memcpy(hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr));
     if (pieces) std::memcpy(pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4);
     if (cellidx) std::memcpy(cellidx, m.tile_cellidx.data(), m.tile_cellidx.size());
-    if (fluid && !m.tile_fluid.empty()) std::memcpy(fluid, m.tile_fluid.data(), m.tile_fluid.size() * 4);
     if (n_fluid_ghosts) *n_fluid_ghosts = (int64_t)m.fluid_leaf.size();
     if (fluid_leaf) std::memcpy(fluid_leaf, m.fluid_leaf.data(), m.fluid_leaf.size() * 8);
     return UFS_DVM_OK;

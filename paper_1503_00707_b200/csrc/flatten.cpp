@@ -556,12 +556,10 @@ struct TileBuild {
     uint32_t pieces[8][256];
     int np[8];
     uint8_t cidx[8][TILE_CELLS][CELLIDX_BYTES];
-    int32_t fluid[TILE_CELLS][24];
     bool any_fluid;
 };
 bool make_tile(const FlatMesh& m, int64_t s0, int nc, int pmax, TileBuild& t) {
     t.any_fluid = false;
-    for (int c = 0; c < TILE_CELLS; c++) for (int k = 0; k < 24; k++) t.fluid[c][k] = -1;
     for (int o = 0; o < 8; o++) {
         int np = 0;
         auto piece = [&](uint32_t code) -> int {
@@ -575,6 +573,7 @@ bool make_tile(const FlatMesh& m, int64_t s0, int nc, int pmax, TileBuild& t) {
         for (int c = 0; c < nc; c++) {
             const CellRec& r = m.recs[s0 + c];
             uint8_t flags = 0;
+            uint32_t fmask = 0;   // bit 4a + k: source k on axis a is a fluid leaf
             for (int a = 0; a < 3; a++) {
                 const int dir = 2 * a + (1 - ((o >> a) & 1));  // xi_a > 0: data comes from the low side
                 const int cnt = r.src[dir][1] >= 0 ? 4 : 1;
@@ -583,23 +582,21 @@ bool make_tile(const FlatMesh& m, int64_t s0, int nc, int pmax, TileBuild& t) {
                     const int32_t code = r.src[dir][k];
                     const int kind = code >> SRC_SHIFT;
                     const int64_t idx = code & SRC_INDEX_MASK;
-                    uint8_t e;
-                    if (kind == SRC_FLUID) {
-                        e = IDX_FLUID; flags |= CIDX_FLUID; t.any_fluid = true;
-                        t.fluid[c][dir * 4 + k] = (int32_t)idx;
-                    } else {
-                        uint32_t pc;
-                        if (kind == SRC_SLAB) pc = (uint32_t)(idx * 8 + o);
-                        else if (kind == SRC_MIRROR) pc = (uint32_t)(idx * 8 + (o ^ (1 << a)));  // specular: mirrored octant of the own slab
-                        else pc = PIECE_TABLE | (uint32_t)(idx * 8 + o);
-                        const int pi = piece(pc);
-                        if (pi >= IDX_FLUID) return false;
-                        e = (uint8_t)pi;
-                    }
-                    t.cidx[o][c][4 + 4 * a + k] = e;
+                    uint32_t pc;
+                    if (kind == SRC_SLAB) pc = (uint32_t)(idx * 8 + o);
+                    else if (kind == SRC_MIRROR) pc = (uint32_t)(idx * 8 + (o ^ (1 << a)));  // specular: mirrored octant of the own slab
+                    else if (kind == SRC_FLUID) {   // the producer warps write its factor rows into the slot (nothing is copied)
+                        pc = PIECE_FLUID | (uint32_t)(idx * 8 + o);
+                        flags |= CIDX_FLUID; fmask |= 1u << (4 * a + k); t.any_fluid = true;
+                    } else pc = PIECE_TABLE | (uint32_t)(idx * 8 + o);
+                    const int pi = piece(pc);
+                    if (pi >= IDX_NONE) return false;
+                    t.cidx[o][c][4 + 4 * a + k] = (uint8_t)pi;
                 }
             }
             t.cidx[o][c][1] = flags;
+            t.cidx[o][c][2] = (uint8_t)(fmask & 0xff);
+            t.cidx[o][c][3] = (uint8_t)(fmask >> 8);
         }
         if (np > pmax) return false;
         t.np[o] = np;
@@ -666,8 +663,8 @@ int build_remap(const FlatMesh& o, const FlatMesh& nw, RemapPlan& plan, std::str
 
 void build_tiles(FlatMesh& m, int pmax) {
     m.tile_pmax = pmax;
-    m.tiles.clear(); m.tile_pieces.clear(); m.tile_cellidx.clear(); m.tile_fluid.clear();
-    const bool has_fluid = !m.fluid.empty();
+    m.tiles.clear(); m.tile_pieces.clear(); m.tile_cellidx.clear();
+    m.tiles_have_fluid = !m.fluid.empty();
     // pass 1 (serial, cheap): tile boundaries; pass 2: fill the arrays
     std::vector<int64_t> start; std::vector<int> count;
     TileBuild* tb = new TileBuild;
@@ -687,7 +684,6 @@ void build_tiles(FlatMesh& m, int pmax) {
     m.tiles.assign(nt, TileHdr{});
     m.tile_pieces.assign((size_t)nt * 8 * pmax, 0u);
     m.tile_cellidx.assign((size_t)nt * 8 * TILE_CELLS * CELLIDX_BYTES, IDX_NONE);
-    if (has_fluid) m.tile_fluid.assign((size_t)nt * TILE_CELLS * 24, -1);
 #pragma omp parallel
     {
         TileBuild* t = new TileBuild;
@@ -702,7 +698,6 @@ void build_tiles(FlatMesh& m, int pmax) {
                 std::memcpy(&m.tile_pieces[((size_t)i * 8 + o) * pmax], t->pieces[o], (size_t)t->np[o] * 4);
                 std::memcpy(&m.tile_cellidx[((size_t)i * 8 + o) * TILE_CELLS * CELLIDX_BYTES], t->cidx[o], TILE_CELLS * CELLIDX_BYTES);
             }
-            if (has_fluid) std::memcpy(&m.tile_fluid[(size_t)i * TILE_CELLS * 24], t->fluid, sizeof t->fluid);
         }
         delete t;
     }

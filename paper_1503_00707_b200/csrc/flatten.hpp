@@ -72,12 +72,16 @@ struct FluidGhost {          // frozen Maxwellian of a FLUID leaf, separable fac
 // cell, which piece is its own chunk and which pieces are its upwind sources on each axis -- the first-order stencil
 // records of PAPER.md:113-115, deduplicated per tile.
 constexpr int TILE_CELLS = 8;
-constexpr uint32_t PIECE_TABLE = 0x80000000u;  // piece code: bit 31 = inflow ghost table, bits 0..30 = (slab or table) * 8 + octant
+constexpr uint32_t PIECE_TABLE = 0x80000000u;  // piece code: bit 31 = inflow ghost table, bits 0..29 = (slab, table or fluid ghost) * 8 + octant
+constexpr uint32_t PIECE_FLUID = 0x40000000u;  // ... bit 30 = a fluid ghost: the producer warps write its factor rows, nothing is copied
+constexpr uint32_t PIECE_INDEX = 0x3fffffffu;
 constexpr uint8_t IDX_NONE = 0xFF;             // cell index table: unused source
-constexpr uint8_t IDX_FLUID = 0xFE;            // ... source is a fluid leaf (computed, not copied)
-constexpr int CELLIDX_BYTES = 16;              // per (tile, octant, cell): [0] own piece, [1] flags, [4+4a+k] source k on axis a
+constexpr int CELLIDX_BYTES = 16;              // per (tile, octant, cell): [0] own piece, [1] flags, [2..3] fluid mask, [4+4a+k] source k on axis a
 constexpr uint8_t CIDX_FOUR = 0x07;            // flags bits 0..2: axis a has four (finer) sources, each weighted 1/4
-constexpr uint8_t CIDX_FLUID = 0x08;           // flags bit 3: some source of the cell is IDX_FLUID
+constexpr uint8_t CIDX_FLUID = 0x08;           // flags bit 3: some source of the cell is a fluid leaf (which: bit 4a + k of bytes [2..3])
+// A fluid piece holds, as doubles, the 12 x factors g_x[rank] of the octant's x sign, then the row factors
+// b[row] = amp g_z g_y of the stage's NRP rows: the leaf's Maxwellian at (row, rank) is b[row] g_x[rank] (separable, G13).
+constexpr int FLUID_PIECE_GX = 0, FLUID_PIECE_B = 12;
 struct TileHdr {                               // 32 bytes
     int32_t s0, nc;                            // first slab, cells
     uint8_t np[8];                             // pieces per octant
@@ -132,7 +136,7 @@ struct FlatMesh {
     std::vector<TileHdr> tiles;
     std::vector<uint32_t> tile_pieces;      // [n_tiles][8 octants][tile_pmax]
     std::vector<uint8_t> tile_cellidx;      // [n_tiles][8 octants][TILE_CELLS][CELLIDX_BYTES]
-    std::vector<int32_t> tile_fluid;        // [n_tiles][TILE_CELLS][24] fluid ghost of source k of direction d (d*4+k), or empty
+    bool tiles_have_fluid = false;          // some piece is a fluid ghost: the kernel's FLUID instantiation
 };
 
 // Returns UFS_DVM_OK or an error code with a message in `err`.

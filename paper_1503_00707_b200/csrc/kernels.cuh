@@ -48,7 +48,7 @@ struct StepParams {
     const TileHdr* tile_hdr;        // [n_tiles]
     const uint32_t* tile_pieces;    // [n_tiles][8][tile_pmax]
     const uint8_t* tile_cellidx;    // [n_tiles][8][TILE_CELLS][CELLIDX_BYTES]
-    const int32_t* tile_fluid;      // [n_tiles][TILE_CELLS][24] or NULL
+    int32_t tiles_have_fluid;       // some piece is a fluid ghost (k_tiles' FLUID instantiation)
     int32_t n_tiles, tile_pmax;
 };
 

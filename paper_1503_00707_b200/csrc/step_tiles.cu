@@ -39,8 +39,8 @@ constexpr int REGS_PROD = 80, REGS_CONS = 144;
 constexpr int TSLOTS = 3;               // tile header slots
 constexpr int DESC_BYTES = TILE_CELLS * CELLIDX_BYTES + 16;   // cell index tables, then the stage's first piece slot
 constexpr int THDR_NEXT = 36;           // tile header: TileHdr (32 B), tile id (or -1: stop), next tile id,
-constexpr int THDR_FLUID = 64;          //   fluid ghost ids int32[8][24],
-constexpr int THDR_TAB = 896;           //   factor tables [8][tabn] of the storage type
+constexpr int THDR_TAB = 64;            //   factor tables [8][tabn] of the storage type
+constexpr int FLUID_PIECE_N = FLUID_PIECE_B + NRP;   // doubles of a fluid piece: 12 x factors, then NRP row factors
 constexpr int RED_DOUBLES = TILE_CELLS * 3 * SUMS_STRIDE;     // partial sums: [cell][16-lane group][36]
 
 struct TilesSmem { uint32_t ring, desc, thdr, red, full, empty, tinfo, ttab, tempty, total, thdr_bytes; };
@@ -74,20 +74,17 @@ __device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
     halve<5, 1>(v, lane);
 }
 
-// Upwind values of a kinetic/fluid face (reading G13): pointwise Maxwellian of the fluid leaf's frozen
-// moments from its separable factors; j = 16-byte vector of the row, (ry, rz) = ranks of |xi_y|, |xi_z|.
-template <typename T>
-__device__ __forceinline__ void fluid_row_vec(const StepParams& p, int ghost, int o, int j, int ry, int rz, T (&v)[V16<T>::N]) {
-    constexpr int VEC = V16<T>::N;
+// Element e of the fluid piece of ghost `ghost` for sign group o and row block q (flatten.hpp: FLUID_PIECE_*): the
+// separable factors of the pointwise Maxwellian of a FLUID leaf's frozen moments (reading G13).  The row
+// factor is formed exactly as the host forms the ghost's velocity sums (api.cu: ghost_state_sums): amp g_z g_y.
+__device__ __forceinline__ double fluid_piece_element(const StepParams& p, int ghost, int o, int q, int e) {
     const FluidGhost* g = p.fluid + ghost;
+    if (e < FLUID_PIECE_B) return g->g[0][(o & 1) ? p.nh[0] + e : p.nh[0] - 1 - e];
+    const int row = q * NRP + (e - FLUID_PIECE_B);
+    const int ry = row % p.nh[1], rz = row / p.nh[1];
     const int kz = ((o >> 2) & 1) ? p.nh[2] + rz : p.nh[2] - 1 - rz;
     const int ky = ((o >> 1) & 1) ? p.nh[1] + ry : p.nh[1] - 1 - ry;
-    const double b = g->amp * g->g[2][kz] * g->g[1][ky];
-#pragma unroll
-    for (int i = 0; i < VEC; i++) {
-        const int kx = (o & 1) ? p.nh[0] + j * VEC + i : p.nh[0] - 1 - j * VEC - i;
-        v[i] = (T)(b * g->g[0][kx]);
-    }
+    return g->amp * g->g[2][kz] * g->g[1][ky];
 }
 
 template <typename T, bool FLUID, bool SUMS_ONLY>
@@ -175,11 +172,9 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     smbar_arrive(sb + o_tinfo + 8u * ts);
                     const uint32_t tb = sb + o_ttab + 8u * ts;
                     const uint32_t tab_bytes = (p.collide && !SUMS_ONLY && tile >= 0) ? (uint32_t)(nc * tabn) * (uint32_t)sizeof(T) : 0u;
-                    const uint32_t fl_bytes = (FLUID && tile >= 0) ? (uint32_t)(TILE_CELLS * 24 * 4) : 0u;
-                    if (tab_bytes + fl_bytes) {
-                        smbar_arrive_expect_tx(tb, tab_bytes + fl_bytes);
-                        if (tab_bytes) sbulk_g2s(hdr + THDR_TAB, reinterpret_cast<const T*>(p.tabs) + (size_t)s0 * tabn, tab_bytes, tb);
-                        if (fl_bytes) sbulk_g2s(hdr + THDR_FLUID, p.tile_fluid + (size_t)tile * TILE_CELLS * 24, fl_bytes, tb);
+                    if (tab_bytes) {
+                        smbar_arrive_expect_tx(tb, tab_bytes);
+                        sbulk_g2s(hdr + THDR_TAB, reinterpret_cast<const T*>(p.tabs) + (size_t)s0 * tabn, tab_bytes, tb);
                     } else {
                         smbar_arrive(tb);
                     }
@@ -223,23 +218,64 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     const int slot = k % NSTG;
                     const uint32_t fb = sb + o_full + 8u * slot;
                     const uint32_t dsc = sb + o_desc + slot * DESC_BYTES;
-                    const int mine = npk > w ? (npk + 3 - w) >> 2 : 0;   // pieces this warp copies
-                    // (test hook, UFS_DVM_TEST_STALL: one producer warp withholds its arrival on the fourth stage; the
-                    // consumers' wait then runs into the watchdog, include/ufs_dvm.h)
-                    if (lane == 0 && !(p.smap[11] && k == 3 && w == 1)) {
-                        if (w == 0) ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
-                        const uint32_t extra = (w == 0 && !SUMS_ONLY) ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u;
-                        smbar_arrive_expect_tx(fb, (uint32_t)mine * PB + extra);
-                        if (extra) sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), extra, fb);
-                    }
-                    __syncwarp();
-                    if (my_piece < npk) {
-                        const uint32_t c = SUMS_ONLY ? (uint32_t)((s0 + my_piece) * 8 + o) : code[o];
-                        const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
-                                       + (size_t)(c & ~PIECE_TABLE) * (size_t)CH + (size_t)q * (NRP * THX);
+                    if constexpr (!FLUID) {
+                        const int mine = npk > w ? (npk + 3 - w) >> 2 : 0;   // pieces this warp copies
+                        // (test hook, UFS_DVM_TEST_STALL: one producer warp withholds its arrival on the fourth stage; the
+                        // consumers' wait then runs into the watchdog, include/ufs_dvm.h)
+                        if (lane == 0 && !(p.smap[11] && k == 3 && w == 1)) {
+                            if (w == 0) ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
+                            const uint32_t extra = (w == 0 && !SUMS_ONLY) ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u;
+                            smbar_arrive_expect_tx(fb, (uint32_t)mine * PB + extra);
+                            if (extra) sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), extra, fb);
+                        }
+                        __syncwarp();
+                        if (my_piece < npk) {
+                            const uint32_t c = SUMS_ONLY ? (uint32_t)((s0 + my_piece) * 8 + o) : code[o];
+                            const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
+                                           + (size_t)(c & PIECE_INDEX) * (size_t)CH + (size_t)q * (NRP * THX);
+                            int ps = head + my_piece;
+                            if (ps >= NP) ps -= NP;
+                            sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
+                        }
+                    } else {
+                        // meshes with FLUID leaves: a piece is a bulk copy, or a fluid ghost's factor rows, which the warp
+                        // writes itself: the elements of all its fluid pieces of the stage are spread over the 32 lanes
+                        const bool have = my_piece < npk;
+                        const uint32_t c = have ? code[o] : 0u;
+                        const bool is_fl = have && (c & PIECE_FLUID);
                         int ps = head + my_piece;
                         if (ps >= NP) ps -= NP;
-                        sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
+                        if (lane == 0 && w == 0) {
+                            ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
+                            sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), (uint32_t)(TILE_CELLS * CELLIDX_BYTES), fb);
+                        }
+                        if (have && !is_fl) {
+                            const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
+                                           + (size_t)(c & PIECE_INDEX) * (size_t)CH + (size_t)q * (NRP * THX);
+                            sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
+                        }
+                        const uint32_t fm = __ballot_sync(0xffffffffu, is_fl);
+                        const int n_copy = __popc(__ballot_sync(0xffffffffu, have && !is_fl));
+                        const int n_el = __popc(fm) * FLUID_PIECE_N;
+                        for (int e0 = 0; e0 < n_el; e0 += 32) {
+                            const int e = e0 + lane;
+                            const bool valid = e < n_el;
+                            const int pi = valid ? e / FLUID_PIECE_N : 0;
+                            const int sl = (int)__fns(fm, 0, pi + 1);                 // lane that owns the pi-th fluid piece
+                            const uint32_t cc = __shfl_sync(0xffffffffu, c, sl);
+                            const int pss = __shfl_sync(0xffffffffu, ps, sl);
+                            if (valid) {
+                                const int idx = e - pi * FLUID_PIECE_N;
+                                const double v = fluid_piece_element(p, (int)((cc & PIECE_INDEX) >> 3), o, q, idx);
+                                asm volatile("st.shared.f64 [%0], %1;" ::"r"(sb + (uint32_t)pss * PB + 8u * (uint32_t)idx), "d"(v) : "memory");
+                            }
+                        }
+                        __syncwarp();
+                        // one arrival per producer warp: it publishes the rows written above (release) and announces the bytes
+                        // of the copies issued above (a copy that completes first only runs the count negative: the phase
+                        // cannot complete before this arrival).  (Test hook: see the other branch.)
+                        if (lane == 0 && !(p.smap[11] && k == 3 && w == 1))
+                            smbar_arrive_expect_tx(fb, (uint32_t)n_copy * PB + (w == 0 ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u));
                     }
                     head += npk;
                     if (head >= NP) head -= NP;
@@ -408,7 +444,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     } else {
                         // 2:1 faces towards finer leaves (four sources, each weighted 1/4: reading G3) and / or fluid leaves
                         const uint32_t words[3] = {ix.y, ix.z, ix.w};
-                        const int* fl = reinterpret_cast<const int*>(smem_raw + hdr + THDR_FLUID) + c * 24;
+                        const uint32_t fmask = FLUID ? (ix.x >> 16) : 0u;   // bit 4a + m: source m on axis a is a fluid ghost
                         // unrolled where every source is a piece (same-box A/B: config 4 -4 %, config 3' -3 %); kept rolled
                         // where fluid sources are formed from global factor tables (unrolled: config 5' +40 %)
 #pragma unroll(FLUID ? 1 : RV)
@@ -418,14 +454,20 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
 #pragma unroll
                             for (int a = 0; a < 3; a++) {
                                 const int nsrc = (flags >> a) & 1u ? 4 : 1;
-                                const int dir = 2 * a + (1 - ((o >> a) & 1));
 #pragma unroll
                                 for (int i = 0; i < VEC; i++) S[a][i] = T(0);
                                 for (int m = 0; m < nsrc; m++) {
                                     const uint32_t b = (words[a] >> (8 * m)) & 0xffu;
                                     T v[VEC];
-                                    if (FLUID && b == IDX_FLUID) fluid_row_vec<T>(p, fl[dir * 4 + m], o, j, ry, rz, v);
-                                    else lds16(addr_of(b) + j * VEC, v);
+                                    if (FLUID && ((fmask >> (4 * a + m)) & 1u)) {
+                                        // the fluid leaf's Maxwellian at (row, rank) = row factor x x factor (flatten.hpp)
+                                        int ps = head + (int)b;
+                                        if (ps >= NP) ps -= NP;
+                                        const double* fp = reinterpret_cast<const double*>(smem_raw + (uint32_t)ps * PB);
+                                        const double bb = fp[FLUID_PIECE_B + rr];
+#pragma unroll
+                                        for (int i = 0; i < VEC; i++) v[i] = (T)(bb * fp[FLUID_PIECE_GX + j * VEC + i]);
+                                    } else lds16(addr_of(b) + j * VEC, v);
 #pragma unroll
                                     for (int i = 0; i < VEC; i++) S[a][i] += v[i];
                                 }
@@ -597,8 +639,8 @@ cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& 
     cudaError_t e = launch_prep(storage, p, st);
     if (e != cudaSuccess) return e;
     if (storage == UFS_STORE_F32)
-        return p.tile_fluid ? launch_tiles_t<float, true, false>(plan, p, st, true) : launch_tiles_t<float, false, false>(plan, p, st, true);
-    return p.tile_fluid ? launch_tiles_t<double, true, false>(plan, p, st, true) : launch_tiles_t<double, false, false>(plan, p, st, true);
+        return p.tiles_have_fluid ? launch_tiles_t<float, true, false>(plan, p, st, true) : launch_tiles_t<float, false, false>(plan, p, st, true);
+    return p.tiles_have_fluid ? launch_tiles_t<double, true, false>(plan, p, st, true) : launch_tiles_t<double, false, false>(plan, p, st, true);
 }
 
 // sums[n_kin][SUMS_STRIDE] of an f the caller has just written: the same kernel, own chunks only, no store

@@ -12,6 +12,8 @@ from paper_1503_00707_b200 import inputs
 from tests.helpers import periodic_case, random_tree
 
 PIECE_TABLE = 0x80000000
+PIECE_FLUID = 0x40000000      # a fluid ghost: its Maxwellian is formed on chip from factor rows, nothing is copied
+PIECE_INDEX = 0x3fffffff
 
 
 def _host(case, storage=None):
@@ -43,10 +45,15 @@ def _transport_through_tiles(case, h, f0_rows, dt):
         s0, nc = int(T["s0"][t]), int(T["nc"][t])
         for o in range(8):
             def chunk(code):
+                c = code & PIECE_INDEX
                 if code & PIECE_TABLE:
-                    c = code & 0x7fffffff
                     return tables[c // 8][c % 8]
-                return f[code // 8, code % 8]
+                if code & PIECE_FLUID:
+                    assert c % 8 == o
+                    leaf = int(T["fluid_leaf"][c // 8])
+                    assert case.kind[leaf] == inputs.CELL_FLUID
+                    return inputs.maxwellian_canonical(case, case.fluid_moments[leaf][None, :])[0][vel_of_slot].reshape(8, CH)[o]
+                return f[c // 8, c % 8]
             pcs = T["pieces"][t, o]
             for c in range(nc):
                 ix = T["cellidx"][t, o, c]
@@ -62,14 +69,11 @@ def _transport_through_tiles(case, h, f0_rows, dt):
                     for k in range(4 if four else 1):
                         b = int(ix[4 + 4 * a + k])
                         assert b != 0xFF
-                        if b == 0xFE:
-                            d = 2 * a + (1 - ((o >> a) & 1))
-                            leaf = int(T["fluid_leaf"][T["fluid"][t, c, d * 4 + k]])
-                            assert case.kind[leaf] == inputs.CELL_FLUID
-                            g = inputs.maxwellian_canonical(case, case.fluid_moments[leaf][None, :])[0][vel_of_slot].reshape(8, CH)[o]
-                            src = src + g
-                        else:
-                            src = src + chunk(int(pcs[b]))
+                        is_fluid = bool(int(pcs[b]) & PIECE_FLUID)
+                        # the per-cell fluid mask (bytes 2..3, bit 4a + k) and flag bit 3 say the same
+                        assert bool(((int(ix[2]) | (int(ix[3]) << 8)) >> (4 * a + k)) & 1) == is_fluid
+                        assert not is_fluid or (ix[1] & 0x08)
+                        src = src + chunk(int(pcs[b]))
                     if not four:
                         assert all(int(x) == 0xFF for x in ix[5 + 4 * a: 8 + 4 * a])
                     acc = acc + dth * w * (0.25 if four else 1.0) * src.reshape(nh, nh, nh)
