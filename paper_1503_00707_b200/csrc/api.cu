@@ -124,6 +124,10 @@ StepParams make_params(ufs_dvm_t h, double dt) {
             p.xpow[0][r] = x; p.xpow[1][r] = x * x; p.xpow[2][r] = x * x * x;
             p.xf[r] = (float)x;
         }
+        for (int r = 0; r < 16; r++) {
+            p.yabs[r] = r < v.nh[1] ? v.xi[1][v.nh[1] + r] : 0.0;
+            p.zabs[r] = r < v.nh[2] ? v.xi[2][v.nh[2] + r] : 0.0;
+        }
     }
     return p;
 }

@@ -43,6 +43,7 @@ struct StepParams {
     // row kernel (step_rows.cu): |xi_x| of the x ranks and its powers (uniform operands, constant bank)
     double xpow[3][16];         // [r-1][rank] = |xi_x|^r, r = 1..3
     float xf[16];               // |xi_x| in fp32
+    double yabs[16], zabs[16];  // tile kernel: |xi_y|, |xi_z| by rank (constant bank: with 225 KB of shared memory L1 is ~3 KB)
     uint32_t smap[12];          // row / tile kernel: its shared-memory map (byte offsets), computed by the launcher
     // tile kernel (step_tiles.cu): the tile records of the flattener
     const TileHdr* tile_hdr;        // [n_tiles]

@@ -293,7 +293,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
     const int c = ct / NRP, rr = ct % NRP;
     const int gi = rr >> 4;                          // 16-lane group of the cell
     const int ry = rr % p.nh[1], rzl = rr / p.nh[1]; // rank of |xi_y|; rank of |xi_z| inside the row block
-    const double ay = p.vel->xi[1][p.nh[1] + ry];
+    const double ay = p.yabs[ry];
     const uint32_t rowoff = (uint32_t)rr * ROWB;
     const int triple = (warp - N_PROD) / 3;          // three warps share two cells: named barrier 1 + triple
     int k = 0;
@@ -326,7 +326,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
         double* const red = reinterpret_cast<double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)(c * 3 + gi) * SUMS_STRIDE;
         for (int q = 0; q < NQ; q++) {
             const int rz = q * (NRP / p.nh[1]) + rzl;
-            const double az = p.vel->xi[2][p.nh[2] + rz];
+            const double az = p.zabs[rz];
             const T cz = (T)(omd * az);
             const T base = (T)(om1 - omd * (ay + az));
             // ... and the own-value coefficients B - Cx_k:  f' = (B - Cx_k) f + Cx_k fX + Cy fY + Cz fZ + W gx_k
