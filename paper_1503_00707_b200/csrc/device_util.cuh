@@ -111,6 +111,16 @@ __device__ __forceinline__ void smbar_wait(uint32_t bar, uint32_t parity) {
         if (globaltimer_ns() - t0 > UFS_WAIT_TIMEOUT_NS) __trap();
     }
 }
+// The same wait for a warp that is in no hurry (a producer waiting for a ring slot, several stages ahead of the
+// consumers): sleeps between polls so that it does not take issue slots and power from the warps that do the work.
+__device__ __forceinline__ void smbar_wait_relaxed(uint32_t bar, uint32_t parity) {
+    if (smbar_try_wait(bar, parity)) return;
+    const unsigned long long t0 = globaltimer_ns();
+    while (!smbar_try_wait(bar, parity)) {
+        __nanosleep(256);
+        if (globaltimer_ns() - t0 > UFS_WAIT_TIMEOUT_NS) __trap();
+    }
+}
 __device__ __forceinline__ void sbulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");

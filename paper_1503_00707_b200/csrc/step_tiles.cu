@@ -210,7 +210,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     const int npk = (int)((np_cur >> (8 * o)) & 0xffull);
                     // ring space: piece slots and the barrier pair of stage k
                     while (k - r >= NSTG || alloc + (uint32_t)npk - rel > (uint32_t)NP) {
-                        smbar_wait(sb + o_empty + 8u * (r % NSTG), (uint32_t)((r / NSTG) & 1));
+                        smbar_wait_relaxed(sb + o_empty + 8u * (r % NSTG), (uint32_t)((r / NSTG) & 1));
                         rel += (uint32_t)(((r_prev ? np_prev : np_cur) >> (8 * (rq & 7))) & 0xffull);
                         r++;
                         if (++rq == 8 * NQ) { rq = 0; r_prev = false; }
