@@ -169,7 +169,7 @@ struct LbmUnroll<T, Q, Q> {
 };
 
 template <typename T, int Q>
-__global__ void __launch_bounds__(128) k_lbm_step(const LbmParams p) {
+__global__ void __launch_bounds__(128, Q == 19 ? 8 : 6) k_lbm_step(const LbmParams p) {
     const T* __restrict__ fin = reinterpret_cast<const T*>(p.f_in);
     T* __restrict__ fout = reinterpret_cast<T*>(p.f_out);
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
