@@ -441,6 +441,56 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 s3_ = fma(p.xpow[2][kk], d, s3_);
                             }
                         }
+                    } else if (FLUID && (flags & CIDX_FOUR) == 0u) {
+                        // one source per axis, some of them fluid leaves (the common cell under a kinetic/fluid mask): a
+                        // piece is read, a fluid source is row factor x x factor from its mini-piece (flatten.hpp)
+                        const uint32_t fmask = ix.x >> 16;
+                        const uint32_t bsrc[3] = {ix.y & 0xffu, ix.z & 0xffu, ix.w & 0xffu};
+                        const bool isfl[3] = {(fmask & 0x001u) != 0u, (fmask & 0x010u) != 0u, (fmask & 0x100u) != 0u};
+                        const T* ap[3];
+                        const double* fq[3];
+                        double bb[3];
+#pragma unroll
+                        for (int a = 0; a < 3; a++) {
+                            int ps = head + (int)bsrc[a];
+                            if (ps >= NP) ps -= NP;
+                            fq[a] = reinterpret_cast<const double*>(smem_raw + (uint32_t)ps * PB);
+                            ap[a] = reinterpret_cast<const T*>(smem_raw + (uint32_t)ps * PB + rowoff);
+                            bb[a] = isfl[a] ? fq[a][FLUID_PIECE_B + rr] : 0.0;
+                        }
+#pragma unroll
+                        for (int j = 0; j < RV; j++) {
+                            T own[VEC], S[3][VEC], out[VEC];
+                            lds16(a_own + j * VEC, own);
+#pragma unroll
+                            for (int a = 0; a < 3; a++) {
+                                if (isfl[a]) {
+#pragma unroll
+                                    for (int i = 0; i < VEC; i++) S[a][i] = (T)(bb[a] * fq[a][FLUID_PIECE_GX + j * VEC + i]);
+                                } else lds16(ap[a] + j * VEC, S[a]);
+                            }
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                out[i] = base * own[i] + cx * (S[0][i] - own[i]) + cy * S[1][i] + cz * S[2][i];
+                            }
+                            if (p.collide) {
+                                T gx[VEC];
+                                lds16(gxrow + j * VEC, gx);
+#pragma unroll
+                                for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
+                            }
+                            stg16_cs(gdst + j * VEC, out);
+#pragma unroll
+                            for (int i = 0; i < VEC; i++) {
+                                const int kk = j * VEC + i;
+                                const double d = (double)out[i];
+                                s0_ += d;
+                                s1_ = fma(p.xpow[0][kk], d, s1_);
+                                s2_ = fma(p.xpow[1][kk], d, s2_);
+                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                            }
+                        }
                     } else {
                         // 2:1 faces towards finer leaves (four sources, each weighted 1/4: reading G3) and / or fluid leaves
                         const uint32_t words[3] = {ix.y, ix.z, ix.w};
