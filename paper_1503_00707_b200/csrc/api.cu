@@ -37,6 +37,7 @@ struct ufs_dvm_s {
     TileHdr* d_tile_hdr = nullptr;
     uint32_t* d_tile_pieces = nullptr;
     uint8_t* d_tile_cellidx = nullptr;
+    double* d_fluid_pieces = nullptr;
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
@@ -116,6 +117,7 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.tile_pieces = h->d_tile_pieces;
     p.tile_cellidx = h->d_tile_cellidx;
     p.tiles_have_fluid = h->mesh.tiles_have_fluid ? 1 : 0;
+    p.fluid_pieces = h->d_fluid_pieces;
     p.n_tiles = (int32_t)h->mesh.tiles.size();
     p.tile_pmax = h->mesh.tile_pmax;
     if (v.fast) {
@@ -308,6 +310,12 @@ static int create_device(ufs_dvm_t h, void* f_dev[2], void* cuda_stream) {
         if ((rc = upload(h, &h->d_tile_hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr), "upload tile headers"))) return rc;
         if ((rc = upload(h, &h->d_tile_pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4, "upload tile piece lists"))) return rc;
         if ((rc = upload(h, &h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), "upload tile index tables"))) return rc;
+        if (m.tiles_have_fluid) {
+            std::vector<double> fp;
+            tiles_fluid_pieces(m, fp);
+            if ((rc = upload(h, &h->d_fluid_pieces, fp.data(), fp.size() * sizeof(double), "upload fluid pieces"))) return rc;
+            CU(cudaStreamSynchronize(h->stream), "upload");   // fp dies here
+        }
     }
     if (h->plan.ring >= 2 && m.n_kin > 0) {
         const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
@@ -443,7 +451,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
-        cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx);
+        cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_fluid_pieces);
         cudaFree(h->d_check);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);

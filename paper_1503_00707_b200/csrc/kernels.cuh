@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <vector>
 
 #include "flatten.hpp"
 
@@ -50,6 +51,7 @@ struct StepParams {
     const uint32_t* tile_pieces;    // [n_tiles][8][tile_pmax]
     const uint8_t* tile_cellidx;    // [n_tiles][8][TILE_CELLS][CELLIDX_BYTES]
     int32_t tiles_have_fluid;       // some piece is a fluid ghost (k_tiles' FLUID instantiation)
+    const double* fluid_pieces;     // [n_fluid_ghosts * 8][row blocks][64] the fluid ghosts' factor rows (tiles_fluid_pieces)
     int32_t n_tiles, tile_pmax;
 };
 
@@ -91,6 +93,7 @@ cudaError_t launch_check_sums(int storage, const StepLaunch& plan, const StepPar
 
 // step_tiles.cu: the same step over tiles of up to eight consecutive slabs (shared upwind chunks on chip)
 bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax);
+void tiles_fluid_pieces(const FlatMesh& m, std::vector<double>& out);   // host: the table behind StepParams::fluid_pieces
 cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 

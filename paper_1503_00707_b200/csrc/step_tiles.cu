@@ -41,6 +41,7 @@ constexpr int DESC_BYTES = TILE_CELLS * CELLIDX_BYTES + 16;   // cell index tabl
 constexpr int THDR_NEXT = 36;           // tile header: TileHdr (32 B), tile id (or -1: stop), next tile id,
 constexpr int THDR_TAB = 64;            //   factor tables [8][tabn] of the storage type
 constexpr int FLUID_PIECE_N = FLUID_PIECE_B + NRP;   // doubles of a fluid piece: 12 x factors, then NRP row factors
+constexpr int FLUID_PIECE_STRIDE = 64;               // ... padded to 512 bytes in the device table of all fluid pieces
 constexpr int RED_DOUBLES = TILE_CELLS * 3 * SUMS_STRIDE;     // partial sums: [cell][16-lane group][36]
 
 struct TilesSmem { uint32_t ring, desc, thdr, red, full, empty, tinfo, ttab, tempty, total, thdr_bytes; };
@@ -72,19 +73,6 @@ __device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
     halve<18, 4>(v, lane);
     halve<9, 2>(v, lane);
     halve<5, 1>(v, lane);
-}
-
-// Element e of the fluid piece of ghost `ghost` for sign group o and row block q (flatten.hpp: FLUID_PIECE_*): the
-// separable factors of the pointwise Maxwellian of a FLUID leaf's frozen moments (reading G13).  The row
-// factor is formed exactly as the host forms the ghost's velocity sums (api.cu: ghost_state_sums): amp g_z g_y.
-__device__ __forceinline__ double fluid_piece_element(const StepParams& p, int ghost, int o, int q, int e) {
-    const FluidGhost* g = p.fluid + ghost;
-    if (e < FLUID_PIECE_B) return g->g[0][(o & 1) ? p.nh[0] + e : p.nh[0] - 1 - e];
-    const int row = q * NRP + (e - FLUID_PIECE_B);
-    const int ry = row % p.nh[1], rz = row / p.nh[1];
-    const int kz = ((o >> 2) & 1) ? p.nh[2] + rz : p.nh[2] - 1 - rz;
-    const int ky = ((o >> 1) & 1) ? p.nh[1] + ry : p.nh[1] - 1 - ry;
-    return g->amp * g->g[2][kz] * g->g[1][ky];
 }
 
 template <typename T, bool FLUID, bool SUMS_ONLY>
@@ -238,44 +226,32 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
                         }
                     } else {
-                        // meshes with FLUID leaves: a piece is a bulk copy, or a fluid ghost's factor rows, which the warp
-                        // writes itself: the elements of all its fluid pieces of the stage are spread over the 32 lanes
+                        // meshes with FLUID leaves: a piece is a bulk copy of a chunk's rows, or of a fluid ghost's factor rows
+                        // for this sign group and row block (512 bytes from the table tiles_fluid_pieces() built)
                         const bool have = my_piece < npk;
                         const uint32_t c = have ? code[o] : 0u;
                         const bool is_fl = have && (c & PIECE_FLUID);
-                        int ps = head + my_piece;
-                        if (ps >= NP) ps -= NP;
-                        if (lane == 0 && w == 0) {
-                            ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
-                            sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), (uint32_t)(TILE_CELLS * CELLIDX_BYTES), fb);
-                        }
-                        if (have && !is_fl) {
-                            const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
-                                           + (size_t)(c & PIECE_INDEX) * (size_t)CH + (size_t)q * (NRP * THX);
-                            sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
-                        }
-                        const uint32_t fm = __ballot_sync(0xffffffffu, is_fl);
+                        const int n_fl = __popc(__ballot_sync(0xffffffffu, is_fl));
                         const int n_copy = __popc(__ballot_sync(0xffffffffu, have && !is_fl));
-                        const int n_el = __popc(fm) * FLUID_PIECE_N;
-                        for (int e0 = 0; e0 < n_el; e0 += 32) {
-                            const int e = e0 + lane;
-                            const bool valid = e < n_el;
-                            const int pi = valid ? e / FLUID_PIECE_N : 0;
-                            const int sl = (int)__fns(fm, 0, pi + 1);                 // lane that owns the pi-th fluid piece
-                            const uint32_t cc = __shfl_sync(0xffffffffu, c, sl);
-                            const int pss = __shfl_sync(0xffffffffu, ps, sl);
-                            if (valid) {
-                                const int idx = e - pi * FLUID_PIECE_N;
-                                const double v = fluid_piece_element(p, (int)((cc & PIECE_INDEX) >> 3), o, q, idx);
-                                asm volatile("st.shared.f64 [%0], %1;" ::"r"(sb + (uint32_t)pss * PB + 8u * (uint32_t)idx), "d"(v) : "memory");
-                            }
+                        if (lane == 0 && !(p.smap[11] && k == 3 && w == 1)) {   // (test hook: see the other branch)
+                            if (w == 0) ssts_i32(dsc + TILE_CELLS * CELLIDX_BYTES, head);
+                            const uint32_t extra = w == 0 ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u;
+                            smbar_arrive_expect_tx(fb, (uint32_t)n_copy * PB + (uint32_t)n_fl * (uint32_t)(FLUID_PIECE_STRIDE * 8) + extra);
+                            if (extra) sbulk_g2s(dsc, p.tile_cellidx + ((size_t)tile * 8 + o) * (TILE_CELLS * CELLIDX_BYTES), extra, fb);
                         }
                         __syncwarp();
-                        // one arrival per producer warp: it publishes the rows written above (release) and announces the bytes
-                        // of the copies issued above (a copy that completes first only runs the count negative: the phase
-                        // cannot complete before this arrival).  (Test hook: see the other branch.)
-                        if (lane == 0 && !(p.smap[11] && k == 3 && w == 1))
-                            smbar_arrive_expect_tx(fb, (uint32_t)n_copy * PB + (w == 0 ? (uint32_t)(TILE_CELLS * CELLIDX_BYTES) : 0u));
+                        if (have) {
+                            int ps = head + my_piece;
+                            if (ps >= NP) ps -= NP;
+                            if (is_fl) {
+                                const double* src = p.fluid_pieces + ((size_t)(c & PIECE_INDEX) * (size_t)NQ + (size_t)q) * FLUID_PIECE_STRIDE;
+                                sbulk_g2s(sb + (uint32_t)ps * PB, src, (uint32_t)(FLUID_PIECE_STRIDE * 8), fb);
+                            } else {
+                                const T* src = ((c & PIECE_TABLE) ? reinterpret_cast<const T*>(p.tables) : fin)
+                                               + (size_t)(c & PIECE_INDEX) * (size_t)CH + (size_t)q * (NRP * THX);
+                                sbulk_g2s(sb + (uint32_t)ps * PB, src, PB, fb);
+                            }
+                        }
                     }
                     head += npk;
                     if (head >= NP) head -= NP;
@@ -657,6 +633,30 @@ cudaError_t launch_tiles_t(const StepLaunch& plan, const StepParams& p, cudaStre
 }
 
 }  // namespace
+
+// The fluid pieces of every fluid ghost: [ghost * 8 + octant][row block][FLUID_PIECE_STRIDE] doubles -- the 12 x factors of
+// the sign group's x sign, then the NRP row factors amp g_z g_y of the block's rows (flatten.hpp; the product in the
+// order in which the host forms the ghost's velocity sums, api.cu: ghost_state_sums).  12 KB per fluid ghost for 24^3.
+void tiles_fluid_pieces(const FlatMesh& m, std::vector<double>& out) {
+    const VelLayout& v = m.vel;
+    const int nq = v.nh[1] * v.nh[2] / NRP;
+    out.assign(m.fluid.size() * 8 * (size_t)nq * FLUID_PIECE_STRIDE, 0.0);
+#pragma omp parallel for schedule(static)
+    for (int64_t gi = 0; gi < (int64_t)m.fluid.size(); gi++) {
+        const FluidGhost& g = m.fluid[gi];
+        for (int o = 0; o < 8; o++)
+            for (int q = 0; q < nq; q++) {
+                double* d = out.data() + (((size_t)gi * 8 + o) * nq + q) * FLUID_PIECE_STRIDE;
+                for (int e = 0; e < THX; e++) d[FLUID_PIECE_GX + e] = g.g[0][(o & 1) ? v.nh[0] + e : v.nh[0] - 1 - e];
+                for (int rr = 0; rr < NRP; rr++) {
+                    const int row = q * NRP + rr, ry = row % v.nh[1], rz = row / v.nh[1];
+                    const int kz = ((o >> 2) & 1) ? v.nh[2] + rz : v.nh[2] - 1 - rz;
+                    const int ky = ((o >> 1) & 1) ? v.nh[1] + ry : v.nh[1] - 1 - ry;
+                    d[FLUID_PIECE_B + rr] = g.amp * g.g[2][kz] * g.g[1][ky];
+                }
+            }
+    }
+}
 
 // Launch geometry of the tile kernel, or false if the velocity grid does not fit it (12 x-ranks per row, whole row
 // blocks of 48 rows, octant layout); *pmax = pieces a tile may list per octant (two stages must fit the ring).
