@@ -312,7 +312,7 @@ static int create_device(ufs_dvm_t h, void* f_dev[2], void* cuda_stream) {
         if ((rc = upload(h, &h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), "upload tile index tables"))) return rc;
         if (m.tiles_have_fluid) {
             std::vector<double> fp;
-            tiles_fluid_pieces(m, fp);
+            tiles_fluid_pieces(m, h->storage, fp);
             if ((rc = upload(h, &h->d_fluid_pieces, fp.data(), fp.size() * sizeof(double), "upload fluid pieces"))) return rc;
             CU(cudaStreamSynchronize(h->stream), "upload");   // fp dies here
         }

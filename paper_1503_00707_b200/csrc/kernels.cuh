@@ -93,7 +93,7 @@ cudaError_t launch_check_sums(int storage, const StepLaunch& plan, const StepPar
 
 // step_tiles.cu: the same step over tiles of up to eight consecutive slabs (shared upwind chunks on chip)
 bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax);
-void tiles_fluid_pieces(const FlatMesh& m, std::vector<double>& out);   // host: the table behind StepParams::fluid_pieces
+void tiles_fluid_pieces(const FlatMesh& m, int storage, std::vector<double>& out);   // host: the table behind StepParams::fluid_pieces
 cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
 cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 

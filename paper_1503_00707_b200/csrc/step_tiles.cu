@@ -27,8 +27,17 @@
 namespace ufs {
 namespace {
 
-constexpr int NRP = 48;                 // rows of a piece
 constexpr int THX = 12;                 // values of a row (nh_x)
+// Geometry of a piece by storage type.  fp32: 48 rows of 48 bytes, one consumer thread per row.  fp64: a row is 96 bytes,
+// and one row per lane read with 16-byte loads hits only four distinct 16-byte offsets modulo 128 in a quarter-warp
+// (96 r mod 128): a 2-way shared-memory bank conflict on every load, 46 % of the wavefronts (profiles/r2_full_config2.md).
+// So fp64 takes 24 rows per piece and one thread per HALF row: lanes are 48 bytes apart as for fp32 (conflict-free), a
+// piece is 2304 bytes for both types, and the ring is as many stages deep for fp64 as for fp32.
+template <typename T> struct Geo { static constexpr int NRP = 48, HALVES = 1; };
+template <> struct Geo<double> { static constexpr int NRP = 24, HALVES = 2; };
+constexpr int PIECE_BYTES = 2304;       // = NRP * THX * sizeof(T) for both
+constexpr int CELL_THREADS = 48;        // consumer threads of a cell = NRP * HALVES
+__host__ __device__ constexpr int nrp_of(size_t elem) { return elem == 8 ? 24 : 48; }
 constexpr int N_PROD = 4;               // producer warps: warps 0..3
 constexpr int N_CONS = 12;              // consumer warps: warps 4..15
 constexpr int NSTG = 8;                 // stage barrier pairs / stage descriptors
@@ -40,7 +49,6 @@ constexpr int TSLOTS = 3;               // tile header slots
 constexpr int DESC_BYTES = TILE_CELLS * CELLIDX_BYTES + 16;   // cell index tables, then the stage's first piece slot
 constexpr int THDR_NEXT = 36;           // tile header: TileHdr (32 B), tile id (or -1: stop), next tile id,
 constexpr int THDR_TAB = 64;            //   factor tables [8][tabn] of the storage type
-constexpr int FLUID_PIECE_N = FLUID_PIECE_B + NRP;   // doubles of a fluid piece: 12 x factors, then NRP row factors
 constexpr int FLUID_PIECE_STRIDE = 64;               // ... padded to 512 bytes in the device table of all fluid pieces
 constexpr int RED_DOUBLES = TILE_CELLS * 3 * SUMS_STRIDE;     // partial sums: [cell][16-lane group][36]
 
@@ -48,7 +56,8 @@ struct TilesSmem { uint32_t ring, desc, thdr, red, full, empty, tinfo, ttab, tem
 __host__ __device__ inline TilesSmem tiles_map(size_t elem, int np, int tabn) {
     TilesSmem s;
     size_t off = 0;
-    s.ring = 0; off += (size_t)np * NRP * THX * elem;
+    s.ring = 0; off += (size_t)np * PIECE_BYTES;
+    (void)elem;
     s.desc = (uint32_t)off; off += (size_t)NSTG * DESC_BYTES;
     off = (off + 127) & ~(size_t)127;
     s.thdr_bytes = (uint32_t)((THDR_TAB + (size_t)TILE_CELLS * tabn * elem + 127) & ~(size_t)127);
@@ -65,7 +74,6 @@ __host__ __device__ inline TilesSmem tiles_map(size_t elem, int np, int tabn) {
 
 template <typename T> __device__ __forceinline__ T tx_of(const StepParams& p, int k);
 template <> __device__ __forceinline__ float tx_of<float>(const StepParams& p, int k) { return p.xf[k]; }
-template <> __device__ __forceinline__ double tx_of<double>(const StepParams& p, int k) { return p.xpow[0][k]; }
 
 // halving butterfly over the 16 lanes of a group: 36 -> 18 -> 9 -> 5 -> 3 values per lane (stream_common.cuh: halve)
 __device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
@@ -77,7 +85,10 @@ __device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
 
 template <typename T, bool FLUID, bool SUMS_ONLY>
 __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepParams p) {
-    constexpr int VEC = V16<T>::N, RV = THX / VEC;
+    constexpr int NRP = Geo<T>::NRP, HALVES = Geo<T>::HALVES;
+    constexpr int XT = THX / HALVES;                    // x ranks of a consumer thread: the whole row, or half of it
+    constexpr int VEC = V16<T>::N, RV = XT / VEC;       // ... = three 16-byte vectors for both storage types
+    static_assert(NRP * THX * sizeof(T) == PIECE_BYTES && NRP * HALVES == CELL_THREADS && RV == 3, "piece geometry");
     constexpr bool PACKED = sizeof(T) == 4 && !SUMS_ONLY;   // fp32 storage: packed two-value arithmetic in the row update
     constexpr uint32_t ROWB = THX * sizeof(T);          // bytes of a row
     constexpr uint32_t PB = NRP * ROWB;                 // bytes of a piece
@@ -266,12 +277,23 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
     // =============================================================== consumer warps: thread = (cell c, row r of the piece)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_CONS));
     const int ct = tid - N_PROD * 32;
-    const int c = ct / NRP, rr = ct % NRP;
-    const int gi = rr >> 4;                          // 16-lane group of the cell
+    const int c = ct / CELL_THREADS, hr = ct % CELL_THREADS;
+    const int rr = hr / HALVES;                      // row of the piece
+    const int k0 = (hr % HALVES) * XT;               // first x rank of this thread
+    const int gi = hr >> 4;                          // 16-lane group of the cell
     const int ry = rr % p.nh[1], rzl = rr / p.nh[1]; // rank of |xi_y|; rank of |xi_z| inside the row block
     const double ay = p.yabs[ry];
-    const uint32_t rowoff = (uint32_t)rr * ROWB;
+    const uint32_t rowoff = (uint32_t)rr * ROWB + (uint32_t)k0 * (uint32_t)sizeof(T);   // = 48 hr: lanes 48 bytes apart
     const int triple = (warp - N_PROD) / 3;          // three warps share two cells: named barrier 1 + triple
+    // fp64 (half rows): the thread's six x ranks are fixed for the whole run, |xi_x| of them stays in registers
+    double txr[HALVES == 2 ? XT : 1];
+    if constexpr (HALVES == 2) {
+#pragma unroll
+        for (int i = 0; i < XT; i++) {
+            txr[i] = p.xpow[0][k0 + i];
+            asm volatile("" : "+d"(txr[i]));
+        }
+    }
     int k = 0;
     for (int n = 0;; n++) {
         const int ts = n % TSLOTS;
@@ -332,6 +354,26 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                 const int slot = k % NSTG;
                 smbar_wait(sb + o_full + 8u * slot, (uint32_t)((k / NSTG) & 1));
                 double s0_ = 0, s1_ = 0, s2_ = 0, s3_ = 0;
+                // the row's x sums s_r += |xi_x,k|^r d.  fp32: powers from the constant bank (k is a compile-time index);
+                // fp64 half rows: Horner with the thread's own |xi_x| (registers; `_dyn`: k known at run time only)
+                auto row_sums = [&](double d, int kk) {
+                    if constexpr (HALVES == 1) {
+                        s0_ += d; s1_ = fma(p.xpow[0][kk], d, s1_); s2_ = fma(p.xpow[1][kk], d, s2_); s3_ = fma(p.xpow[2][kk], d, s3_);
+                    } else {
+                        const double x = txr[kk], t1 = x * d, t2 = x * t1;
+                        s0_ += d; s1_ += t1; s2_ += t2; s3_ = fma(x, t2, s3_);
+                    }
+                };
+                auto row_sums_dyn = [&](double d, int kk) {
+                    if constexpr (HALVES == 1) {
+                        s0_ += d; s1_ = fma(p.xpow[0][kk], d, s1_); s2_ = fma(p.xpow[1][kk], d, s2_); s3_ = fma(p.xpow[2][kk], d, s3_);
+                    } else {
+                        const double x = p.xpow[0][k0 + kk], t1 = x * d, t2 = x * t1;
+                        s0_ += d; s1_ += t1; s2_ += t2; s3_ = fma(x, t2, s3_);
+                    }
+                };
+                auto xk = [&](int kk) -> T { if constexpr (HALVES == 1) return tx_of<T>(p, kk); else return (T)txr[kk]; };
+                auto xk_dyn = [&](int kk) -> T { if constexpr (HALVES == 1) return tx_of<T>(p, kk); else return (T)p.xpow[0][k0 + kk]; };
                 if (active) {
                     const unsigned char* dsc = smem_raw + o_desc + slot * DESC_BYTES;
                     const int head = *reinterpret_cast<const int*>(dsc + TILE_CELLS * CELLIDX_BYTES);
@@ -345,9 +387,9 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     };
                     const T* a_own = addr_of(ix.x & 0xffu);
                     const uint32_t flags = (ix.x >> 8) & 0xffu;
-                    T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX;
+                    T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX + k0;
                     T wb = T(0);
-                    const T* gxrow = tab + (o & 1) * nhp;
+                    const T* gxrow = tab + (o & 1) * nhp + k0;
                     if (!SUMS_ONLY) wb = ((o & 4) ? wgz[1] : wgz[0]) * ((o & 2) ? wgy[1] : wgy[0]);
                     // packed path: the relaxation term is always added; with collisions off W = 0 multiplies the own row
                     // (finite values) instead of a factor table nobody wrote
@@ -359,12 +401,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             lds16(a_own + j * VEC, own);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
-                                const int kk = j * VEC + i;
-                                const double d = (double)own[i];
-                                s0_ += d;
-                                s1_ = fma(p.xpow[0][kk], d, s1_);
-                                s2_ = fma(p.xpow[1][kk], d, s2_);
-                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                                row_sums((double)own[i], j * VEC + i);
                             }
                         }
                     } else if (flags == 0) {
@@ -396,7 +433,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             } else {
 #pragma unroll
                                 for (int i = 0; i < VEC; i++) {
-                                    const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                    const T cx = sxc * xk(j * VEC + i);
                                     out[i] = base * own[i] + cx * (X[i] - own[i]) + cy * Y[i] + cz * Z[i];
                                 }
                                 if (p.collide) {
@@ -409,12 +446,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             stg16_cs(gdst + j * VEC, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
-                                const int kk = j * VEC + i;
-                                const double d = (double)out[i];
-                                s0_ += d;
-                                s1_ = fma(p.xpow[0][kk], d, s1_);
-                                s2_ = fma(p.xpow[1][kk], d, s2_);
-                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                                row_sums((double)out[i], j * VEC + i);
                             }
                         }
                     } else if (FLUID && (flags & CIDX_FOUR) == 0u) {
@@ -442,12 +474,12 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             for (int a = 0; a < 3; a++) {
                                 if (isfl[a]) {
 #pragma unroll
-                                    for (int i = 0; i < VEC; i++) S[a][i] = (T)(bb[a] * fq[a][FLUID_PIECE_GX + j * VEC + i]);
+                                    for (int i = 0; i < VEC; i++) S[a][i] = (T)(bb[a] * fq[a][FLUID_PIECE_GX + k0 + j * VEC + i]);
                                 } else lds16(ap[a] + j * VEC, S[a]);
                             }
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
-                                const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                const T cx = sxc * xk(j * VEC + i);
                                 out[i] = base * own[i] + cx * (S[0][i] - own[i]) + cy * S[1][i] + cz * S[2][i];
                             }
                             if (p.collide) {
@@ -459,12 +491,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             stg16_cs(gdst + j * VEC, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
-                                const int kk = j * VEC + i;
-                                const double d = (double)out[i];
-                                s0_ += d;
-                                s1_ = fma(p.xpow[0][kk], d, s1_);
-                                s2_ = fma(p.xpow[1][kk], d, s2_);
-                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                                row_sums((double)out[i], j * VEC + i);
                             }
                         }
                     } else {
@@ -492,7 +519,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                         const double* fp = reinterpret_cast<const double*>(smem_raw + (uint32_t)ps * PB);
                                         const double bb = fp[FLUID_PIECE_B + rr];
 #pragma unroll
-                                        for (int i = 0; i < VEC; i++) v[i] = (T)(bb * fp[FLUID_PIECE_GX + j * VEC + i]);
+                                        for (int i = 0; i < VEC; i++) v[i] = (T)(bb * fp[FLUID_PIECE_GX + k0 + j * VEC + i]);
                                     } else lds16(addr_of(b) + j * VEC, v);
 #pragma unroll
                                     for (int i = 0; i < VEC; i++) S[a][i] += v[i];
@@ -519,7 +546,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             } else {
 #pragma unroll
                                 for (int i = 0; i < VEC; i++) {
-                                    const T cx = sxc * tx_of<T>(p, j * VEC + i);
+                                    const T cx = sxc * (FLUID ? xk_dyn(j * VEC + i) : xk(j * VEC + i));   // (rolled loop in the fluid instantiation)
                                     out[i] = base * own[i] + cx * (S[0][i] - own[i]) + cy * S[1][i] + cz * S[2][i];
                                 }
                                 if (p.collide) {
@@ -532,12 +559,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                             stg16_cs(gdst + j * VEC, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
-                                const int kk = j * VEC + i;
-                                const double d = (double)out[i];
-                                s0_ += d;
-                                s1_ = fma(p.xpow[0][kk], d, s1_);
-                                s2_ = fma(p.xpow[1][kk], d, s2_);
-                                s3_ = fma(p.xpow[2][kk], d, s3_);
+                                if constexpr (FLUID) row_sums_dyn((double)out[i], j * VEC + i); else row_sums((double)out[i], j * VEC + i);
                             }
                         }
                     }
@@ -637,8 +659,9 @@ cudaError_t launch_tiles_t(const StepLaunch& plan, const StepParams& p, cudaStre
 // The fluid pieces of every fluid ghost: [ghost * 8 + octant][row block][FLUID_PIECE_STRIDE] doubles -- the 12 x factors of
 // the sign group's x sign, then the NRP row factors amp g_z g_y of the block's rows (flatten.hpp; the product in the
 // order in which the host forms the ghost's velocity sums, api.cu: ghost_state_sums).  12 KB per fluid ghost for 24^3.
-void tiles_fluid_pieces(const FlatMesh& m, std::vector<double>& out) {
+void tiles_fluid_pieces(const FlatMesh& m, int storage, std::vector<double>& out) {
     const VelLayout& v = m.vel;
+    const int NRP = nrp_of(storage == UFS_STORE_F32 ? 4 : 8);
     const int nq = v.nh[1] * v.nh[2] / NRP;
     out.assign(m.fluid.size() * 8 * (size_t)nq * FLUID_PIECE_STRIDE, 0.0);
 #pragma omp parallel for schedule(static)
@@ -663,6 +686,7 @@ void tiles_fluid_pieces(const FlatMesh& m, std::vector<double>& out) {
 bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax) {
     if (!v.fast || v.nh[0] != THX) return false;
     const int nr = v.nh[1] * v.nh[2];
+    const int NRP = nrp_of(storage == UFS_STORE_F32 ? 4 : 8);
     if (nr % NRP != 0 || NRP % v.nh[1] != 0 || (nr / NRP) * 8 < NSTG) return false;
     for (int a = 0; a < 3; a++)
         if (v.nv[a] > 32) return false;
