@@ -119,3 +119,51 @@ def test_lbm_conserves_mass_on_the_periodic_tree():
     m1 = st.moments()
     st.close()
     assert np.abs(((m1 - m0) * vol).sum(axis=1)).max() <= 1e-13 * (m0[0] * vol).sum()
+
+
+@pytest.mark.gpu
+def test_lbm_on_the_million_leaf_octree_windows_and_conservation():
+    """The bench workload of the LBM variant (D3Q19 on the 1 009 261-leaf periodic config-4 octree, fp64): parity at
+    sampled cells against the oracle on the sub-mesh within S = 3 face rings of each (values outside the domain of
+    dependence cannot reach the sample after S steps; window mode pinned in tests/test_oracle_window_pin.py), then
+    conservation of total mass and momentum over 20 steps."""
+    from oracle.dvm_oracle import Oracle
+    from paper_1503_00707_b200 import harness
+    S = 3
+    case = inputs.lbm_case(inputs.config4(), 19, noise_rel=0.0)
+    st = K.LbmStepper(case)
+    # f(t=0): the equilibrium of the case's (rho, u) fields, formed by the oracle side and handed to the device
+    f0 = LO.initial_f(case)
+    st.load_canonical(f0)
+    mesh = Oracle(case, kn=math.inf)                      # neighbour search of the whole mesh (for the windows)
+    rng = np.random.default_rng(inputs.SEED_BASE + 919)
+    kin = case.kinetic_leaves()
+    picks = []
+    for l in np.unique(case.level[kin]).tolist():
+        ids = kin[case.level[kin] == l]
+        picks.append(rng.choice(ids, 16, replace=False))
+    picks.append(np.array([st.cell_of_row[0], st.cell_of_row[-1]]))
+    centres = np.unique(np.concatenate(picks))
+    row_of_leaf = np.full(case.n_leaves, -1, np.int64); row_of_leaf[kin] = np.arange(kin.size)
+    vol = 8.0 ** (-case.level[kin].astype(np.float64))
+    m0 = st.moments()
+    st.step(case.dt, S)
+    st.sync()
+    f_gpu = st.read_canonical()
+    worst = 0.0
+    for c in centres.tolist():
+        ids = harness.window_leaves(case, c, S, mesh.leaf_neighbours)
+        sub = inputs.sub_case(case, ids); sub.meta = case.meta
+        o = LO.LbmOracle(sub, inputs.lbm_tau(case), window=True)
+        f_ref = o.step(f0[row_of_leaf[ids]], case.dt, S)
+        k = int(np.searchsorted(ids, c))
+        err = np.abs(f_gpu[row_of_leaf[c]] - f_ref[k]).max() / np.abs(f_ref[k]).max()
+        worst = max(worst, err)
+        assert err <= 1e-12, f"leaf {c} (level {case.level[c]}): {err:.3e}"
+    del mesh
+    st.step(case.dt, 20 - S)
+    m1 = st.moments()
+    st.close()
+    tot0, tot1 = (m0 * vol).sum(axis=1), (m1 * vol).sum(axis=1)
+    assert np.all(np.isfinite(m1))
+    assert np.abs(tot1 - tot0).max() <= 1e-12 * tot0[0]
