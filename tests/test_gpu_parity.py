@@ -249,3 +249,20 @@ def test_check_mode_catches_a_forgotten_f_changed(monkeypatch):
         st.sync()
     assert e.value.code == B.EINVAL and "ufs_dvm_f_changed" in str(e.value)
     st.close()
+
+
+@pytest.mark.parametrize("storage", [inputs.STORE_F64, inputs.STORE_F32])
+@pytest.mark.parametrize("nv", [(24, 16, 12), (24, 8, 24)])
+def test_tile_kernel_on_non_cubic_velocity_grids(nv, storage):
+    """k_tiles takes any even symmetric grid with 12 positive x nodes and whole row blocks (48 rows for fp32, 24 for fp64
+    storage); the row-block / half-row arithmetic must not depend on nh_y = nh_z = 12."""
+    lv, ijk = random_tree(np.random.default_rng(21), 1, 3, P, 0.3)
+    case = periodic_case(lv, ijk, nv=nv, vlim=5.0, kn=0.1)
+    case.storage = storage
+    rng = np.random.default_rng(3)
+    f0 = inputs.initial_f(case) * (1 + 0.2 * rng.uniform(-1, 1, (case.n_leaves, case.Nv)))
+    st = B.DvmStepper(case)
+    name = B.ufs_dvm_kernel_name(st.h)
+    st.close()
+    assert name == "k_tiles"
+    check(case, 3, TOL[storage], f0=f0)
