@@ -100,6 +100,20 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps);
  * n, n*ux, n*uy, n*uz, E = (w/2) sum |xi|^2 f  (PAPER.md:237 for the first two). */
 int ufs_dvm_moments(ufs_dvm_t h, double *mom_dev);
 
+/* The same moments of ANY f in this handle's layout, without allocating anything: for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops).  f_dev: DEVICE, [n_kinetic][Nv] elements of the storage type in slab
+ * and slot order (NULL = the current f); mom_dev: DEVICE, [5][n_kinetic] doubles as above; both caller-owned.  The 35
+ * velocity sums per cell that ufs_dvm_moments keeps in a cudaMalloc'ed buffer go, here, through a fixed array in the
+ * library's device image: UFS_DVM_STATIC_MAX_CELLS * 36 doubles = 2.25 MiB, held by every device that loads the library
+ * until the process exits.  More than UFS_DVM_STATIC_MAX_CELLS kinetic cells, a handle whose device is not the current
+ * device, or a velocity grid without the octant layout (odd or asymmetric): UFS_DVM_EINVAL with the reason in
+ * ufs_dvm_last_error, nothing enqueued.  Calls no cudaMalloc / cudaFree and no allocating library routine; two launches on
+ * the handle's stream.  All calls on one device share the array (it keeps the last call's sums; nothing in it has to start
+ * at zero: every number read is written first by the same call), so calls that OVERLAP on the GPU -- handles on different
+ * streams -- race; calls on one stream are ordered.  The carried sums of the step are neither read nor changed. */
+#define UFS_DVM_STATIC_MAX_CELLS 8192
+int ufs_dvm_moments_static(ufs_dvm_t h, const void *f_dev, double *mom_dev);
+
 /* Wait for the stream and report sticky asynchronous errors (ECUDA, ENEWTON). */
 int ufs_dvm_sync(ufs_dvm_t h);
 

@@ -22,7 +22,9 @@ EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_mom
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
            "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan",
            "ufs_dvm_partition", "ufs_dvm_create_part", "ufs_dvm_create_part_host", "ufs_dvm_part_layout", "ufs_dvm_halo",
-           "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done"]
+           "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done", "ufs_dvm_moments_static"]
+
+STATIC_MAX_CELLS = 8192   # UFS_DVM_STATIC_MAX_CELLS of include/ufs_dvm.h
 
 
 class ufs_dvm_desc(C.Structure):
@@ -52,6 +54,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_create_host.argtypes = [C.POINTER(ufs_dvm_desc), C.POINTER(C.c_void_p)]
         L.ufs_dvm_step.argtypes = [vp, C.c_double, C.c_int]
         L.ufs_dvm_moments.argtypes = [vp, vp]
+        L.ufs_dvm_moments_static.argtypes = [vp, vp, vp]
         L.ufs_dvm_sync.argtypes = [vp]
         L.ufs_dvm_destroy.argtypes = [vp]
         L.ufs_dvm_current.argtypes = [vp]
@@ -139,6 +142,10 @@ def ufs_dvm_step(h, dt: float, nsteps: int = 1):
 
 def ufs_dvm_moments(h, mom_dev_ptr: int):
     _check(h, lib().ufs_dvm_moments(h, C.c_void_p(mom_dev_ptr)))
+
+
+def ufs_dvm_moments_static(h, f_dev_ptr: Optional[int], mom_dev_ptr: int):
+    _check(h, lib().ufs_dvm_moments_static(h, C.c_void_p(f_dev_ptr), C.c_void_p(mom_dev_ptr)))
 
 
 def ufs_dvm_sync(h):
@@ -411,6 +418,16 @@ class DvmStepper:
     def moments(self) -> np.ndarray:
         """[5, n_kinetic] in Case row order: n, n ux, n uy, n uz, E."""
         ufs_dvm_moments(self.h, self.mom.data_ptr())
+        ufs_dvm_sync(self.h)
+        m = self.mom.cpu().numpy()
+        out = np.empty_like(m)
+        out[:, self.row_of_slab] = m
+        return out
+
+    def moments_static(self, f=None) -> np.ndarray:
+        """The same moments through ufs_dvm_moments_static (no allocation in the library: its sums go through the fixed
+        array of STATIC_MAX_CELLS cells); `f`: a device tensor in the handle's layout, default the current f."""
+        ufs_dvm_moments_static(self.h, None if f is None else f.data_ptr(), self.mom.data_ptr())
         ufs_dvm_sync(self.h)
         m = self.mom.cpu().numpy()
         out = np.empty_like(m)

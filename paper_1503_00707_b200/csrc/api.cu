@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -726,3 +727,58 @@ const char* ufs_dvm_kernel_name(ufs_dvm_t h) {
 const char* ufs_dvm_last_error(ufs_dvm_t h) { return h ? h->err.c_str() : "null handle"; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------- ufs_dvm_moments_static: moments without any allocation
+// For callers that cannot allocate (CUDA graph capture, tight serving loops): the sums pass (k_sums) writes the 35
+// velocity sums of every cell of the caller's f into a FIXED array in the library's device image instead of a
+// cudaMalloc'ed buffer, and k_moments_from_sums reads them from there.  Every device that loads the library holds the
+// array (UFS_DVM_STATIC_MAX_CELLS * 36 doubles = 2.25 MiB) until the process exits.  All calls on a device share it:
+// calls that overlap on the GPU (different streams) race.  Nothing in it has to start at zero: k_sums writes all 36
+// numbers of each cell before k_moments_from_sums, later on the same stream, reads them.
+static __device__ __align__(256) double g_static_sums[(size_t)UFS_DVM_STATIC_MAX_CELLS * SUMS_STRIDE];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+double* g_static_sums_ptr[STATIC_MAX_DEVICES] = {};   // the array's DEVICE address, per device ordinal
+std::mutex g_static_mu;
+
+// In host code `g_static_sums` is only a stand-in for the symbol: its device address comes from the runtime, once per
+// device, with that device current.
+cudaError_t static_sums_address(int dev, double** out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_sums_ptr[dev]) {
+        double* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_sums);
+        if (e != cudaSuccess) return e;
+        g_static_sums_ptr[dev] = ptr;
+    }
+    *out = g_static_sums_ptr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int ufs_dvm_moments_static(ufs_dvm_t h, const void* f_dev, double* mom_dev) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (h->mesh.n_kin == 0) return UFS_DVM_OK;
+    if (!mom_dev) return fail(h, UFS_DVM_EINVAL, "mom_dev is NULL");
+    if (h->plan.ring < 2)
+        return fail(h, UFS_DVM_EINVAL, "ufs_dvm_moments_static needs the octant layout of the streaming kernels (even, symmetric velocity grid)");
+    if (h->mesh.n_kin > UFS_DVM_STATIC_MAX_CELLS)
+        return fail(h, UFS_DVM_EINVAL, "ufs_dvm_moments_static: " + std::to_string(h->mesh.n_kin) + " kinetic cells exceed the fixed scratch of UFS_DVM_STATIC_MAX_CELLS = "
+                                           + std::to_string(UFS_DVM_STATIC_MAX_CELLS) + " cells; use ufs_dvm_moments");
+    int dev = -1;
+    CU(cudaGetDevice(&dev), "get device");
+    cudaPointerAttributes attr{};
+    CU(cudaPointerGetAttributes(&attr, h->d_flags), "pointer attributes");
+    if (attr.device != dev || dev < 0 || dev >= STATIC_MAX_DEVICES)
+        return fail(h, UFS_DVM_EINVAL, "ufs_dvm_moments_static: the handle's device (" + std::to_string(attr.device) + ") must be the current device (" + std::to_string(dev) + ")");
+    double* scratch = nullptr;
+    CU(static_sums_address(dev, &scratch), "address of the static scratch");
+    const StepParams p = make_params(h, 1.0);
+    CU(launch_sums(h->storage, h->plan, p, f_dev ? f_dev : h->f[h->cur], scratch, h->stream), "sums kernel launch");
+    CU(launch_moments_from_sums(p, scratch, mom_dev, h->stream), "moments kernel launch");
+    h->launches += 2;
+    return UFS_DVM_OK;
+}
