@@ -157,7 +157,8 @@ def run_partitioned(args):
     import torch.distributed as dist
     from paper_1503_00707_b200 import binding as B
     from paper_1503_00707_b200 import harness
-    from paper_1503_00707_b200.partition import RankStepper, exchange_distributed, exchange_local
+    from paper_1503_00707_b200.partition import (RankStepper, exchange_distributed, exchange_local, setup_push_distributed,
+                                                 setup_push_local, step_pushed_distributed, step_pushed_local)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -173,10 +174,13 @@ def run_partitioned(args):
     desc, keep = B.make_desc(case)
     rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, 0.0)
     mine = list(range(n_ranks)) if emulate else [rank]
-    ranks = [RankStepper(case, rol, r, n_ranks, device=dev) for r in mine]
+    fused = args.fused_exchange
+    ranks = [RankStepper(case, rol, r, n_ranks, device=dev, symmetric=fused and not emulate) for r in mine]
     for st in ranks:
         harness.fill_initial_f_device(st, case)
     stream = ranks[0].stream
+    if fused:
+        setup_push_local(ranks) if emulate else setup_push_distributed(ranks[0])
 
     def exchange():
         if emulate:
@@ -186,15 +190,20 @@ def run_partitioned(args):
 
     def step(k):
         for _ in range(k):
-            exchange()
-            for st in ranks:
-                st.step(case.dt, 1)
+            if fused:          # the step kernel writes the peers' ghost slabs itself; what is left is the ghost sums
+                step_pushed_local(ranks, case.dt) if emulate else step_pushed_distributed(ranks[0], case.dt)
+            else:
+                exchange()
+                for st in ranks:
+                    st.step(case.dt, 1)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    if fused:
+        exchange()             # the ghosts of the very first step
     step(args.warmup)
     barrier()
     launches0 = sum(B.ufs_dvm_launch_count(st.h) for st in ranks)
@@ -207,7 +216,11 @@ def run_partitioned(args):
     launches = sum(B.ufs_dvm_launch_count(st.h) for st in ranks) - launches0
     ev[2].record(stream)                       # the exchange alone (pack, transfer, unpack, ghost sums)
     for _ in range(args.steps):
-        exchange()
+        if fused:
+            for st in ranks:
+                st.halo_done()
+        else:
+            exchange()
     ev[3].record(stream)
     barrier()
     for st in ranks:
@@ -220,8 +233,14 @@ def run_partitioned(args):
     ghosts = sum(st.n_ghost for st in ranks)
     elem = 4 if case.storage == 1 else 8
     cfg = workload_config(case, args)
-    cfg["parallelism"] = (f"{n_ranks} ranks emulated on 1 GPU, one stream (device copy instead of NCCL)" if emulate
-                          else f"{n_ranks} ranks, one GPU each, NCCL send/recv of the packed ghost chunks")
+    if fused:
+        cfg["parallelism"] = (f"{n_ranks} ranks emulated on 1 GPU, one stream; fused exchange: k_tiles stores the boundary cells "
+                              "into the peers' ghost slabs" if emulate
+                              else f"{n_ranks} ranks, one GPU each; fused exchange: k_tiles stores the boundary cells into the "
+                                   "peers' ghost slabs over NVLink (symmetric memory), one stream barrier per step")
+    else:
+        cfg["parallelism"] = (f"{n_ranks} ranks emulated on 1 GPU, one stream (device copy instead of NCCL)" if emulate
+                              else f"{n_ranks} ranks, one GPU each, NCCL send/recv of the packed ghost chunks")
     line = {"metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
@@ -322,6 +341,8 @@ def main():
                     help="N > 1: one partitioned problem over the ranks (ghost exchange) instead of N replicas")
     ap.add_argument("--emulate-ranks", type=int, default=0,
                     help="1 GPU: cut the workload into R ranks on this GPU and step them with the ghost exchange")
+    ap.add_argument("--fused-exchange", action="store_true",
+                    help="partitioned step: the step kernel writes the peers' ghost slabs itself (ufs_dvm_halo_push_setup)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

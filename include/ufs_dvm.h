@@ -236,9 +236,28 @@ int ufs_dvm_halo_unpack(ufs_dvm_t h, int32_t peer, const void *buf_dev);
  * and allow the next ufs_dvm_step. */
 int ufs_dvm_halo_done(ufs_dvm_t h);
 
+/* Fused ghost exchange: step and exchange in ONE kernel over peer memory (PAPER.md:185-187 does the exchange as separate
+ * MPI messages between GPUs; with NVLink / NVSwitch peer access the step kernel can write into the neighbour directly).
+ * After this call every ufs_dvm_step of this handle stores each row of a cell that some peer lists as a ghost cell twice:
+ * into the own next f, and -- for the octants that peer needs -- into that peer's ghost slab of ITS next f, while the rest
+ * of the pass goes on; ufs_dvm_halo_pack / unpack and the transfer between them are then not needed.
+ * Arrays of n_ranks entries (HOST, read during the call), entries of ranks that need nothing from this rank are ignored:
+ * peer_f0[p], peer_f1[p] = rank p's f_dev[0], f_dev[1] as THIS device reaches them (the same process: the pointers
+ * themselves after cudaDeviceEnablePeerAccess; another process: the mappings of cudaIpcOpenMemHandle or of a symmetric
+ * allocation), 16-byte aligned; dest_slab[p][i] = the ghost slab of rank p that holds this rank's i-th send slab, i.e. rank
+ * p's recv_slab list for this rank (ufs_dvm_halo on rank p), n_send entries.
+ * Protocol.  All ranks hold the same ufs_dvm_current (true from creation on; every rank steps once per round).  The first
+ * step still needs one ordinary exchange (pack / transfer / unpack / ufs_dvm_halo_done): nothing has been pushed yet.  From
+ * then on, per step:  ufs_dvm_step(h, dt, 1) on every rank  ->  a barrier ACROSS the ranks' streams (every rank's step kernel
+ * has finished: its ghost slabs are complete, and nobody still reads the buffers the next step will push into)  ->
+ * ufs_dvm_halo_done(h) (ghost sums)  ->  next step.  Double buffering makes that one barrier per step enough.
+ * EINVAL: not a partitioned handle, not the tile kernel, a needed entry is NULL or misaligned, or some cell is needed by
+ * more than four peers (then the pack / unpack exchange serves).  May be called again (new peer addresses). */
+int ufs_dvm_halo_push_setup(ufs_dvm_t h, void *const *peer_f0, void *const *peer_f1, const int32_t *const *dest_slab);
+
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
- * level per cell (8 bytes), 0, 0}; pieces[n_tiles][8][pmax] = source chunk codes: bits 0..29 = index * 8 + octant, the
+ * level per cell (8 bytes), first push entry, eight 4-bit push counts (0, 0 without ufs_dvm_halo_push_setup)}; pieces[n_tiles][8][pmax] = source chunk codes: bits 0..29 = index * 8 + octant, the
  * index being a slab, or an inflow ghost table if bit 31 is set, or a fluid ghost if bit 30 is set (the frozen Maxwellian
  * of a FLUID leaf: nothing is copied, the kernel's producer warps write the leaf's separable factors into
  * the slot); cellidx[n_tiles][8][8][16] bytes = per octant and cell: [0] own piece, [1] flags (bit a: axis a has four

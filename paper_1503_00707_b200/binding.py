@@ -22,7 +22,8 @@ EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_mom
            "ufs_dvm_run_host", "ufs_dvm_launch_count", "ufs_dvm_kernel_info", "ufs_dvm_kernel_name",
            "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan",
            "ufs_dvm_partition", "ufs_dvm_create_part", "ufs_dvm_create_part_host", "ufs_dvm_part_layout", "ufs_dvm_halo",
-           "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done", "ufs_dvm_moments_static"]
+           "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done", "ufs_dvm_moments_static",
+           "ufs_dvm_halo_push_setup"]
 
 STATIC_MAX_CELLS = 8192   # UFS_DVM_STATIC_MAX_CELLS of include/ufs_dvm.h
 
@@ -78,6 +79,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_halo_pack.argtypes = [vp, C.c_int32, vp]
         L.ufs_dvm_halo_unpack.argtypes = [vp, C.c_int32, vp]
         L.ufs_dvm_halo_done.argtypes = [vp]
+        L.ufs_dvm_halo_push_setup.argtypes = [vp, vp, vp, vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
@@ -297,6 +299,17 @@ def ufs_dvm_halo_done(h):
     _check(h, lib().ufs_dvm_halo_done(h))
 
 
+def ufs_dvm_halo_push_setup(h, peer_f0, peer_f1, dest_slab):
+    """peer_f0 / peer_f1: per rank the device address of that rank's f buffers (None for ranks that need nothing from this
+    one); dest_slab: per rank an int32 array (or None)."""
+    n = len(peer_f0)
+    keep = [None if d is None else np.ascontiguousarray(d, np.int32) for d in dest_slab]
+    a0 = (C.c_void_p * n)(*[C.c_void_p(x) for x in peer_f0])
+    a1 = (C.c_void_p * n)(*[C.c_void_p(x) for x in peer_f1])
+    ad = (C.c_void_p * n)(*[C.c_void_p(None if d is None else d.ctypes.data) for d in keep])
+    _check(h, lib().ufs_dvm_halo_push_setup(h, a0, a1, ad))
+
+
 def ufs_dvm_tiles(h) -> dict:
     """The flattener's tile records (see include/ufs_dvm.h); empty arrays if the handle uses another kernel."""
     n, pmax, ng = C.c_int64(), C.c_int32(), C.c_int64()
@@ -309,7 +322,8 @@ def ufs_dvm_tiles(h) -> dict:
                                   cellidx.ctypes.data, C.byref(ng), fluid_leaf.ctypes.data))
     return {"n_tiles": nt, "pmax": pm, "s0": hdr[:, 0].copy(), "nc": hdr[:, 1].copy(),
             "np": hdr[:, 2:4].copy().view(np.uint8).reshape(nt, 8), "level": hdr[:, 4:6].copy().view(np.uint8).reshape(nt, 8),
-            "pieces": pieces, "cellidx": cellidx, "fluid_leaf": fluid_leaf}
+            "pieces": pieces, "cellidx": cellidx, "fluid_leaf": fluid_leaf,
+            "push_first": hdr[:, 6].copy(), "push_counts": hdr[:, 7].copy().view(np.uint32)}
 
 
 def ufs_dvm_run_host(h, f_host_in_ptr: int, f_host_out_ptr: Optional[int], mom_dev_ptr: int, mom_host_ptr: int,

@@ -39,6 +39,7 @@ struct ufs_dvm_s {
     uint32_t* d_tile_pieces = nullptr;
     uint8_t* d_tile_cellidx = nullptr;
     double* d_fluid_pieces = nullptr;
+    PushEntry* d_tile_push = nullptr;   // fused ghost exchange (ufs_dvm_halo_push_setup)
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
@@ -121,6 +122,8 @@ StepParams make_params(ufs_dvm_t h, double dt) {
     p.fluid_pieces = h->d_fluid_pieces;
     p.n_tiles = (int32_t)h->mesh.tiles.size();
     p.tile_pmax = h->mesh.tile_pmax;
+    p.tile_push = h->d_tile_push;
+    p.push_parity = h->cur ^ 1;
     if (v.fast) {
         for (int r = 0; r < v.nh[0] && r < 16; r++) {
             const double x = v.xi[0][v.nh[0] + r];
@@ -453,7 +456,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
         cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_fluid_pieces);
-        cudaFree(h->d_check);
+        cudaFree(h->d_check); cudaFree(h->d_tile_push);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
@@ -682,6 +685,33 @@ int ufs_dvm_halo_done(ufs_dvm_t h) {
         h->launches++;
     }
     h->ghosts_fresh = true;
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer_f1, const int32_t* const* dest_slab) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (!h->mesh.partial) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh");
+    if (h->plan.ring != 4) return fail(h, UFS_DVM_EINVAL, "the fused ghost exchange needs the tile kernel (k_tiles)");
+    if (!peer_f0 || !peer_f1 || !dest_slab) return fail(h, UFS_DVM_EINVAL, "peer_f0, peer_f1 and dest_slab must be arrays of n_ranks entries");
+    FlatMesh& m = h->mesh;
+    const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
+    std::string err;
+    int rc;
+    try {
+        rc = build_push(m, peer_f0, peer_f1, dest_slab, (int64_t)(m.vel.Nv * elem), err);
+    } catch (const std::bad_alloc&) {
+        return fail(h, UFS_DVM_ENOMEM, "out of host memory");
+    }
+    if (rc) return fail(h, rc, err);
+    CU(cudaStreamSynchronize(h->stream), "stream synchronize");   // no step in flight reads the old headers
+    cudaFree(h->d_tile_push);
+    h->d_tile_push = nullptr;
+    if ((rc = upload(h, &h->d_tile_push, m.tile_push.data(), m.tile_push.size() * sizeof(PushEntry), "upload push entries"))) return rc;
+    CU(cudaMemcpyAsync(h->d_tile_hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr), cudaMemcpyHostToDevice, h->stream), "upload tile headers");
+    CU(cudaStreamSynchronize(h->stream), "upload");
+    h->plan.push_on = 1;
     return UFS_DVM_OK;
 }
 

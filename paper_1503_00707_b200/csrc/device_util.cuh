@@ -44,6 +44,9 @@ __device__ __forceinline__ void stg16_cs(float* p, const float (&r)[4]) {
 __device__ __forceinline__ void stg16_cs(double* p, const double (&r)[2]) {
     __stcs(reinterpret_cast<double2*>(p), make_double2(r[0], r[1]));
 }
+// plain 16-byte store (peer memory: the ghost slabs of another rank)
+__device__ __forceinline__ void stg16(float* p, const float (&r)[4]) { *reinterpret_cast<float4*>(p) = make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ void stg16(double* p, const double (&r)[2]) { *reinterpret_cast<double2*>(p) = make_double2(r[0], r[1]); }
 
 // ---- mbarrier + bulk async copy (TMA engine, SASS UBLKCP): producer / consumer ring -----------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

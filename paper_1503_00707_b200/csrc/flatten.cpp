@@ -703,4 +703,46 @@ void build_tiles(FlatMesh& m, int pmax) {
     }
 }
 
+int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_f1, const int32_t* const* dest_slab, int64_t slab_bytes,
+               std::string& err) {
+    if (!m.partial) { err = "fused ghost exchange: not a partitioned mesh"; return UFS_DVM_EINVAL; }
+    if (m.tiles.empty() && m.n_kin > 0) { err = "fused ghost exchange: needs the tile kernel (k_tiles)"; return UFS_DVM_EINVAL; }
+    // per inner slab: the peers that need it
+    std::vector<std::vector<PushEntry>> of_slab(m.n_kin);
+    for (int pr = 0; pr < m.n_ranks; pr++) {
+        const size_t ns = m.send_slab[pr].size();
+        if (ns == 0) continue;
+        if (!peer_f0[pr] || !peer_f1[pr] || !dest_slab[pr]) {
+            err = "fused ghost exchange: rank " + std::to_string(pr) + " needs cells of this rank, but its buffers or slab list are NULL";
+            return UFS_DVM_EINVAL;
+        }
+        for (size_t i = 0; i < ns; i++) {
+            const int32_t s = m.send_slab[pr][i], d = dest_slab[pr][i];
+            if (s < 0 || s >= m.n_kin || d < 0) { err = "fused ghost exchange: slab out of range"; return UFS_DVM_EINVAL; }
+            PushEntry e{};
+            e.dst[0] = (uint64_t)(uintptr_t)peer_f0[pr] + (uint64_t)d * (uint64_t)slab_bytes;
+            e.dst[1] = (uint64_t)(uintptr_t)peer_f1[pr] + (uint64_t)d * (uint64_t)slab_bytes;
+            e.info = m.send_mask[pr][i];
+            if ((e.dst[0] | e.dst[1]) & 15) { err = "fused ghost exchange: peer buffers must be 16-byte aligned"; return UFS_DVM_EINVAL; }
+            of_slab[s].push_back(e);
+        }
+    }
+    m.tile_push.clear();
+    for (TileHdr& t : m.tiles) {
+        t.pad[0] = (int32_t)m.tile_push.size();
+        uint32_t counts = 0;
+        for (int c = 0; c < t.nc; c++) {
+            const std::vector<PushEntry>& v = of_slab[t.s0 + c];
+            if ((int)v.size() > PUSH_PER_CELL_MAX) {
+                err = "fused ghost exchange: a cell is needed by more than " + std::to_string(PUSH_PER_CELL_MAX) + " peers; use ufs_dvm_halo_pack / unpack";
+                return UFS_DVM_EINVAL;
+            }
+            counts |= (uint32_t)v.size() << (4 * c);
+            m.tile_push.insert(m.tile_push.end(), v.begin(), v.end());
+        }
+        t.pad[1] = (int32_t)counts;
+    }
+    return UFS_DVM_OK;
+}
+
 }  // namespace ufs

@@ -90,6 +90,17 @@ struct TileHdr {                               // 32 bytes
 };
 static_assert(sizeof(TileHdr) == 32, "TileHdr must be 32 bytes");
 
+// Fused ghost exchange (build_push): a cell whose chunks a peer rank needs is stored a second time by k_tiles, straight
+// into that peer's ghost slab of the NEXT f.  One entry per (cell, peer); a tile's entries are consecutive, ordered by
+// cell: TileHdr::pad[0] = index of the tile's first entry, pad[1] = eight 4-bit counts (entries of cell c in bits 4c..4c+3).
+constexpr int PUSH_PER_CELL_MAX = 4;           // peers that may need one cell (more: the pack / unpack exchange serves)
+struct PushEntry {                             // 32 bytes
+    uint64_t dst[2];                           // address of the peer's ghost slab in its f buffer 0 / 1 (peer memory)
+    uint32_t info;                             // bits 0..7: octant mask of the chunks the peer needs
+    uint32_t pad[3];
+};
+static_assert(sizeof(PushEntry) == 32, "PushEntry must be 32 bytes");
+
 struct FlatMesh {
     int64_t n_leaves = 0, n_kin = 0;
     // ---- one rank's part of a partitioned mesh (restrict_to_rank).  n_kin counts the rank's own
@@ -137,6 +148,7 @@ struct FlatMesh {
     std::vector<uint32_t> tile_pieces;      // [n_tiles][8 octants][tile_pmax]
     std::vector<uint8_t> tile_cellidx;      // [n_tiles][8 octants][TILE_CELLS][CELLIDX_BYTES]
     bool tiles_have_fluid = false;          // some piece is a fluid ghost: the kernel's FLUID instantiation
+    std::vector<PushEntry> tile_push;       // fused ghost exchange (build_push): the tiles' push entries
 };
 
 // Returns UFS_DVM_OK or an error code with a message in `err`.
@@ -169,5 +181,11 @@ int restrict_to_rank(FlatMesh& m, const int32_t* rank_of_leaf, int my_rank, int 
 // Groups the slabs into tiles whose piece lists hold at most `pmax` pieces per octant (complete sibling octets where
 // the mesh has them, else runs of consecutive slabs) and fills the tile arrays of `m`.
 void build_tiles(FlatMesh& m, int pmax);
+
+// Fused ghost exchange of a partitioned mesh: fills m.tile_push and the pad words of m.tiles from the send lists.  Per peer
+// rank p: peer_f[b][p] = address (as this device reaches it) of rank p's f buffer b, dest_slab[p][i] = the ghost slab of
+// rank p that takes this rank's i-th send slab (rank p's recv_slab list for this rank), slab_bytes = Nv * element size.
+int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_f1, const int32_t* const* dest_slab, int64_t slab_bytes,
+               std::string& err);
 
 }  // namespace ufs

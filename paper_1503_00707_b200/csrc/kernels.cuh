@@ -53,6 +53,9 @@ struct StepParams {
     int32_t tiles_have_fluid;       // some piece is a fluid ghost (k_tiles' FLUID instantiation)
     const double* fluid_pieces;     // [n_fluid_ghosts * 8][row blocks][64] the fluid ghosts' factor rows (tiles_fluid_pieces)
     int32_t n_tiles, tile_pmax;
+    // fused ghost exchange (k_tiles' PUSH instantiation): the tiles' push entries; which of PushEntry::dst[] is the NEXT f
+    const PushEntry* tile_push;
+    int32_t push_parity;
 };
 
 constexpr int SUMS_STRIDE = 36;  // doubles per cell in the sums arrays (35 used)
@@ -64,6 +67,7 @@ struct StepLaunch {
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
     cudaEvent_t ev0, ev1;          // if set: recorded on the stream right before / after the main kernel of the step
     int32_t test_stall;            // UFS_DVM_TEST_STALL was set at creation: k_tiles stalls on purpose (watchdog test)
+    int32_t push_on;               // ufs_dvm_halo_push_setup was called: k_tiles also stores the boundary cells into the peers' ghost slabs
 };
 
 // per-axis table stride (nodes rounded up to a multiple of 4)

@@ -83,7 +83,7 @@ __device__ __forceinline__ void group16_reduce(double (&v)[36], int lane) {
     halve<5, 1>(v, lane);
 }
 
-template <typename T, bool FLUID, bool SUMS_ONLY>
+template <typename T, bool FLUID, bool SUMS_ONLY, bool PUSH = false>
 __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepParams p) {
     constexpr int NRP = Geo<T>::NRP, HALVES = Geo<T>::HALVES;
     constexpr int XT = THX / HALVES;                    // x ranks of a consumer thread: the whole row, or half of it
@@ -321,6 +321,14 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
             }
         }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)(s0 + c) * p.Nv;
+        // fused ghost exchange: the push entries of this thread's cell (flatten.hpp: PushEntry)
+        int pfirst = 0, pcnt = 0;
+        if constexpr (PUSH) {
+            const uint32_t cnts = *reinterpret_cast<const uint32_t*>(smem_raw + hdr + 28);
+            pfirst = *reinterpret_cast<const int*>(smem_raw + hdr + 24);
+            for (int i = 0; i < c; i++) pfirst += (int)((cnts >> (4 * i)) & 15u);
+            pcnt = active ? (int)((cnts >> (4 * c)) & 15u) : 0;
+        }
         double* const red = reinterpret_cast<double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)(c * 3 + gi) * SUMS_STRIDE;
         for (int q = 0; q < NQ; q++) {
             const int rz = q * (NRP / p.nh[1]) + rzl;
@@ -388,6 +396,26 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     const T* a_own = addr_of(ix.x & 0xffu);
                     const uint32_t flags = (ix.x >> 8) & 0xffu;
                     T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX + k0;
+                    // the peers' ghost slabs that take this cell's chunk of octant o: the same row goes there as well
+                    T* pd[PUSH ? PUSH_PER_CELL_MAX : 1];
+                    if constexpr (PUSH) {
+#pragma unroll
+                        for (int e = 0; e < PUSH_PER_CELL_MAX; e++) {
+                            pd[e] = nullptr;
+                            if (e < pcnt) {
+                                const PushEntry* ent = p.tile_push + pfirst + e;
+                                if ((__ldg(&ent->info) >> o) & 1u)
+                                    pd[e] = reinterpret_cast<T*>(__ldg(reinterpret_cast<const unsigned long long*>(ent->dst) + p.push_parity)) + ((int64_t)o * CH + (int64_t)row * THX + k0);
+                            }
+                        }
+                    }
+                    auto push_out = [&](int j, const T (&out)[VEC]) {
+                        if constexpr (PUSH) {
+#pragma unroll
+                            for (int e = 0; e < PUSH_PER_CELL_MAX; e++)
+                                if (pd[e]) stg16(pd[e] + j * VEC, out);
+                        }
+                    };
                     T wb = T(0);
                     const T* gxrow = tab + (o & 1) * nhp + k0;
                     if (!SUMS_ONLY) wb = ((o & 4) ? wgz[1] : wgz[0]) * ((o & 2) ? wgy[1] : wgy[0]);
@@ -444,6 +472,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 }
                             }
                             stg16_cs(gdst + j * VEC, out);
+                            push_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 row_sums((double)out[i], j * VEC + i);
@@ -489,6 +518,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
                             }
                             stg16_cs(gdst + j * VEC, out);
+                            push_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 row_sums((double)out[i], j * VEC + i);
@@ -557,6 +587,7 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 }
                             }
                             stg16_cs(gdst + j * VEC, out);
+                            push_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 if constexpr (FLUID) row_sums_dyn((double)out[i], j * VEC + i); else row_sums((double)out[i], j * VEC + i);
@@ -636,9 +667,9 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
 
 constexpr size_t TILES_SMEM_MAX = 227 * 1024;
 
-template <typename T, bool FLUID, bool SUMS_ONLY>
+template <typename T, bool FLUID, bool SUMS_ONLY, bool PUSH = false>
 cudaError_t launch_tiles_t(const StepLaunch& plan, const StepParams& p, cudaStream_t st, bool timed) {
-    auto kfn = k_tiles<T, FLUID, SUMS_ONLY>;
+    auto kfn = k_tiles<T, FLUID, SUMS_ONLY, PUSH>;
     cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = p.n_tiles < plan.grid ? p.n_tiles : plan.grid;
@@ -712,6 +743,12 @@ cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& 
     if (p.n_kin == 0) return cudaSuccess;
     cudaError_t e = launch_prep(storage, p, st);
     if (e != cudaSuccess) return e;
+    if (plan.push_on) {
+        // fused ghost exchange: the same pass, boundary cells stored a second time into the peers' ghost slabs
+        if (storage == UFS_STORE_F32)
+            return p.tiles_have_fluid ? launch_tiles_t<float, true, false, true>(plan, p, st, true) : launch_tiles_t<float, false, false, true>(plan, p, st, true);
+        return p.tiles_have_fluid ? launch_tiles_t<double, true, false, true>(plan, p, st, true) : launch_tiles_t<double, false, false, true>(plan, p, st, true);
+    }
     if (storage == UFS_STORE_F32)
         return p.tiles_have_fluid ? launch_tiles_t<float, true, false>(plan, p, st, true) : launch_tiles_t<float, false, false>(plan, p, st, true);
     return p.tiles_have_fluid ? launch_tiles_t<double, true, false>(plan, p, st, true) : launch_tiles_t<double, false, false>(plan, p, st, true);

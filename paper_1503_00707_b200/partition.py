@@ -18,7 +18,9 @@ class RankStepper(B.DvmStepper):
     ascending leaf order (self.inner_leaves)."""
 
     def __init__(self, case: Case, rank_of_leaf: np.ndarray, my_rank: int, n_ranks: int, device="cuda:0",
-                 kn: Optional[float] = None, storage: Optional[int] = None, stream=None):
+                 kn: Optional[float] = None, storage: Optional[int] = None, stream=None, symmetric: bool = False, group=None):
+        """symmetric: allocate the two f tensors as symmetric memory of the process group (every rank makes the same
+        calls; sized for the largest rank) so that setup_push_distributed can hand the peers' mappings to the library."""
         import torch
         self.torch = torch
         self.case = case
@@ -34,7 +36,10 @@ class RankStepper(B.DvmStepper):
         self.n_inner, self.n_ghost = lay["n_inner"], lay["n_ghost"]
         n_slabs = self.n_inner + self.n_ghost
         with torch.cuda.device(self.device):
-            self.f = [torch.empty((n_slabs, self.Nv), dtype=self.dtype, device=self.device) for _ in range(2)]
+            if symmetric:
+                self.f, self.f_symm = _symmetric_f(torch, n_slabs, self.Nv, self.dtype, self.device, group)
+            else:
+                self.f = [torch.empty((n_slabs, self.Nv), dtype=self.dtype, device=self.device) for _ in range(2)]
             self.mom = torch.empty((5, max(self.n_inner, 1)), dtype=torch.float64, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self.h = B.ufs_dvm_create_part(desc, rank_of_leaf, my_rank, n_ranks, [t.data_ptr() for t in self.f],
@@ -73,10 +78,32 @@ class RankStepper(B.DvmStepper):
     def halo_done(self):
         B.ufs_dvm_halo_done(self.h)
 
+    def setup_push(self, peer_f, dest_slab):
+        """Switch this rank to the fused ghost exchange (ufs_dvm_halo_push_setup): peer_f[p] = (address of rank p's f
+        buffer 0, of its buffer 1) as this device reaches them, dest_slab[p] = rank p's recv_slab list for this rank;
+        None for ranks that need nothing from this one."""
+        B.ufs_dvm_halo_push_setup(self.h, [None if x is None else x[0] for x in peer_f], [None if x is None else x[1] for x in peer_f],
+                                  dest_slab)
+        self.push = True
+
     def halo_bytes(self):
         """Bytes this rank sends / receives per step."""
         return (sum(t.numel() * t.element_size() for t in self.send_buf.values()),
                 sum(t.numel() * t.element_size() for t in self.recv_buf.values()))
+
+
+def _symmetric_f(torch, n_slabs, Nv, dtype, device, group):
+    """Two f tensors in symmetric memory (torch.distributed._symmetric_memory): same size on every rank (the largest
+    rank's), rendezvous over the group; returns the tensors cut to this rank's slabs and the rendezvous handles."""
+    import torch.distributed as dist
+    import torch.distributed._symmetric_memory as symm
+    most = torch.tensor([n_slabs], dtype=torch.int64, device=device)
+    dist.all_reduce(most, op=dist.ReduceOp.MAX, group=group)
+    rows = max(int(most.item()), 1)
+    name = dist.group.WORLD.group_name if group is None else group.group_name
+    full = [symm.empty((rows, Nv), dtype=dtype, device=device) for _ in range(2)]
+    handles = [symm.rendezvous(t, name) for t in full]
+    return [t[:n_slabs] for t in full], handles
 
 
 def exchange_local(ranks: List[RankStepper]):
@@ -113,4 +140,55 @@ def exchange_distributed(rank: RankStepper, group=None):
                 w.wait()
         for p in rank.peers:
             rank.unpack(p)
+        rank.halo_done()
+
+
+def setup_push_local(ranks: List[RankStepper]):
+    """Fused ghost exchange between ranks emulated on ONE device: every rank's step kernel stores its boundary cells
+    straight into the other ranks' ghost slabs (the same address space: the peers' own pointers)."""
+    n = len(ranks)
+    for r in ranks:
+        peer_f, dest = [None] * n, [None] * n
+        for p in r.peers:
+            if B.ufs_dvm_halo_bytes(r.h, p)[0]:
+                peer_f[p] = (ranks[p].f[0].data_ptr(), ranks[p].f[1].data_ptr())
+                dest[p] = B.ufs_dvm_halo(ranks[p].h, r.my_rank)["recv_slab"]
+        r.setup_push(peer_f, dest)
+
+
+def step_pushed_local(ranks: List[RankStepper], dt: float):
+    """One step of every rank under the fused exchange, ranks emulated on one device and ONE stream: the stream order is
+    the barrier between the step kernels and the ghost sums (no kernel waits on another one)."""
+    for r in ranks:
+        r.step(dt, 1)
+    for r in ranks:
+        r.halo_done()
+
+
+def setup_push_distributed(rank: RankStepper, group=None):
+    """Fused ghost exchange between real ranks of one node.  The two f tensors of `rank` must have been allocated by
+    torch.distributed._symmetric_memory.empty (rank.f_symm = the two rendezvous handles): every rank's buffers are then
+    mapped into every other rank's address space over NVLink, and the peers' recv_slab lists travel once, on the host,
+    by all_gather_object."""
+    import torch.distributed as dist
+    n = rank.n_ranks
+    mine = {p: B.ufs_dvm_halo(rank.h, p)["recv_slab"] for p in rank.peers}
+    everyone = [None] * n
+    dist.all_gather_object(everyone, mine, group=group)
+    peer_f, dest = [None] * n, [None] * n
+    for p in rank.peers:
+        if B.ufs_dvm_halo_bytes(rank.h, p)[0]:
+            peer_f[p] = tuple(int(rank.f_symm[b].buffer_ptrs[p]) for b in range(2))
+            dest[p] = everyone[p][rank.my_rank]
+    rank.setup_push(peer_f, dest)
+    rank.push_token = rank.torch.zeros(1, dtype=rank.torch.int32, device=rank.device)
+
+
+def step_pushed_distributed(rank: RankStepper, dt: float, group=None):
+    """One step under the fused exchange: the step kernel pushes while it computes; a barrier on the stream (NCCL) stands
+    between every rank's step kernel and the ghost sums / the next step."""
+    import torch.distributed as dist
+    with rank.torch.cuda.stream(rank.stream):
+        rank.step(dt, 1)
+        dist.all_reduce(rank.push_token, group=group)     # ordered after the step kernel on this stream, on every rank
         rank.halo_done()

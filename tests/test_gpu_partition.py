@@ -9,14 +9,14 @@ import pytest
 from oracle.dvm_oracle import Oracle
 from paper_1503_00707_b200 import binding as B
 from paper_1503_00707_b200 import inputs
-from paper_1503_00707_b200.partition import RankStepper, exchange_local
+from paper_1503_00707_b200.partition import RankStepper, exchange_local, setup_push_local, step_pushed_local
 from tests.helpers import assert_moments_close, rel_linf
 
 pytestmark = pytest.mark.gpu
 TOL = {inputs.STORE_F64: 1e-12, inputs.STORE_F32: 2e-5}
 
 
-def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0):
+def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False):
     desc, keep = B.make_desc(case)
     rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, w_fluid)
     f0 = inputs.initial_f(case)
@@ -29,10 +29,23 @@ def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0):
         for r in ranks:
             assert B.ufs_dvm_kernel_name(r.h) == "k_tiles"
             r.load_canonical(f0[glob_row[r.inner_leaves]])
-        for _ in range(nsteps):
+        if push:
+            # fused exchange: one ordinary exchange for the first step's ghosts, from then on the step kernels write the
+            # boundary cells into the peers' ghost slabs themselves -- no pack, copy or unpack launch after this point
+            setup_push_local(ranks)
             exchange_local(ranks)
-            for r in ranks:
-                r.step(case.dt, 1)
+            before = [B.ufs_dvm_launch_count(r.h) for r in ranks]
+            for _ in range(nsteps):
+                step_pushed_local(ranks, case.dt)
+            for r, b in zip(ranks, before):
+                per_step = 2 + (1 if r.n_ghost else 0)         # k_prep, k_tiles, ghost sums
+                first = 1 if r.n_inner else 0                  # the sums pass of the initial f
+                assert B.ufs_dvm_launch_count(r.h) - b <= nsteps * per_step + first
+        else:
+            for _ in range(nsteps):
+                exchange_local(ranks)
+                for r in ranks:
+                    r.step(case.dt, 1)
         f = np.empty_like(f0)
         mom = np.empty((5, kin.size))
         for r in ranks:
@@ -110,3 +123,76 @@ def test_partitioned_config3_at_stated_size_four_ranks():
     assert np.all(np.isfinite(f))
     assert rel_linf(f, f_ref) <= 1e-12
     assert_moments_close(mom, o.moments(f_ref), 1e-12)
+
+
+@pytest.mark.parametrize("cfg,n_ranks", [(3, 2), (3, 3), (4, 2), (4, 4), (5, 3)])
+def test_fused_exchange_matches_the_one_domain_oracle(cfg, n_ranks):
+    """ufs_dvm_halo_push_setup: the step kernel stores the boundary cells into the peers' ghost slabs (peer memory; here the
+    ranks share one device) -- 2:1 faces, walls, a SOLID body, the kinetic/fluid mask (k_tiles' FLUID instantiation), fp32."""
+    case = inputs.small(cfg)
+    nsteps = 4
+    f0, f, mom, sent = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=True)
+    o = Oracle(case)
+    f_ref = o.step(f0, case.dt, nsteps)
+    tol = TOL[case.storage]
+    assert np.all(np.isfinite(f))
+    assert rel_linf(f, f_ref) <= tol
+    assert_moments_close(mom, o.moments(f_ref), tol, eps_storage=6e-8 if case.storage == inputs.STORE_F32 else 2.3e-16)
+
+
+def test_fused_exchange_is_bit_equal_to_the_packed_exchange():
+    """The same rows reach the same ghost slabs either way: the two exchanges give bit-identical fields."""
+    case = inputs.small(3)
+    _, f_a, mom_a, _ = _run_partitioned(case, 3, 3)
+    _, f_b, mom_b, _ = _run_partitioned(case, 3, 3, push=True)
+    assert np.array_equal(f_a, f_b)
+    assert np.array_equal(mom_a, mom_b)
+
+
+def test_fused_exchange_push_entries_cover_the_send_lists():
+    case = inputs.small(3)
+    desc, keep = B.make_desc(case)
+    rol = B.ufs_dvm_partition(desc, 3)
+    ranks = [RankStepper(case, rol, r, 3) for r in range(3)]
+    try:
+        setup_push_local(ranks)
+        for r in ranks:
+            t = B.ufs_dvm_tiles(r.h)
+            counts = np.array([[(int(w) >> (4 * c)) & 15 for c in range(8)] for w in t["push_counts"]])
+            assert np.all(counts[np.arange(8)[None, :] >= t["nc"][:, None]] == 0)
+            n_send = sum(B.ufs_dvm_halo(r.h, p)["send_slab"].size for p in range(3))
+            assert counts.sum() == n_send
+            # a tile's entries follow the previous tile's
+            assert np.array_equal(t["push_first"], np.concatenate([[0], np.cumsum(counts.sum(axis=1))[:-1]]))
+            # per cell: as many entries as peers that list it
+            per_slab = np.zeros(r.n_inner, np.int64)
+            for p in range(3):
+                np.add.at(per_slab, B.ufs_dvm_halo(r.h, p)["send_slab"], 1)
+            got = np.zeros(r.n_inner, np.int64)
+            for i in range(t["n_tiles"]):
+                got[t["s0"][i]:t["s0"][i] + t["nc"][i]] = counts[i, :t["nc"][i]]
+            assert np.array_equal(got, per_slab)
+    finally:
+        for r in ranks:
+            r.close()
+
+
+def test_fused_exchange_refuses_what_it_cannot_serve():
+    case = inputs.small(3)
+    desc, keep = B.make_desc(case)
+    st = B.DvmStepper(case)                                   # not partitioned
+    try:
+        with pytest.raises(B.UfsDvmError) as e:
+            B.ufs_dvm_halo_push_setup(st.h, [None], [None], [None])
+        assert e.value.code == B.EINVAL
+    finally:
+        st.close()
+    rol = B.ufs_dvm_partition(desc, 2)
+    ranks = [RankStepper(case, rol, r, 2) for r in range(2)]
+    try:
+        with pytest.raises(B.UfsDvmError) as e:               # rank 1 needs cells of rank 0 but no buffers are given
+            B.ufs_dvm_halo_push_setup(ranks[0].h, [None, None], [None, None], [None, None])
+        assert e.value.code == B.EINVAL and "rank 1" in str(e.value)
+    finally:
+        for r in ranks:
+            r.close()
