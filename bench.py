@@ -208,12 +208,18 @@ def run_partitioned(args):
     barrier()
     launches0 = sum(B.ufs_dvm_launch_count(st.h) for st in ranks)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    for st in ranks:
+        B.ufs_dvm_profile(st.h, True)          # events around each rank's k_tiles launch
     with harness.ClockSampler(index=torch.cuda.current_device()) as clk:
         ev[0].record(stream)
         step(args.steps)
         ev[1].record(stream)
         barrier()
     launches = sum(B.ufs_dvm_launch_count(st.h) for st in ranks) - launches0
+    kernel_ms = 0.0                             # per step: the ranks' streaming kernels one after the other (this process)
+    for st in ranks:
+        kernel_ms += B.ufs_dvm_kernel_ms(st.h)[0]
+        B.ufs_dvm_profile(st.h, False)
     ev[2].record(stream)                       # the exchange alone (pack, transfer, unpack, ghost sums)
     for _ in range(args.steps):
         if fused:
@@ -249,7 +255,8 @@ def run_partitioned(args):
             "halo": {"ranks": n_ranks, "inner_cells_this_process": n_inner, "ghost_cells_this_process": ghosts,
                      "ghost_fraction": ghosts / max(n_inner, 1), "sent_bytes_per_step_this_process": sent,
                      "sent_fraction_of_f": sent / max(n_inner * case.Nv * elem, 1),
-                     "exchange_ms_per_step": ms_x / args.steps, "exchange_share_of_step": ms_x / ms}}
+                     "exchange_ms_per_step": ms_x / args.steps, "exchange_share_of_step": ms_x / ms,
+                     "streaming_kernel_ms_per_step_this_process": kernel_ms}}
     if rank == 0:
         print(json.dumps(line), flush=True)
     for st in ranks:

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of libufs_dvm.so (include/ufs_dvm.h): handle life cycle, uploads of what the
 // flattener built, and the enqueue calls.  No torch types, no exceptions across the boundary.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -40,6 +41,8 @@ struct ufs_dvm_s {
     uint8_t* d_tile_cellidx = nullptr;
     double* d_fluid_pieces = nullptr;
     PushEntry* d_tile_push = nullptr;   // fused ghost exchange (ufs_dvm_halo_push_setup)
+    TileHdr* d_ghost_tiles = nullptr;   // partitioned mesh, tile kernel: the ghost slabs in runs of eight (their sums pass)
+    int64_t n_ghost_tiles = 0;
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
@@ -266,6 +269,20 @@ int ufs_dvm_create_part(const ufs_dvm_desc* desc, const int32_t* rank_of_leaf, i
             if ((rc = upload(h, dir ? &h->d_recv_chunks[pr] : &h->d_send_chunks[pr], chunks.data(), chunks.size() * 4, "upload halo chunk lists"))) return rc;
             CU(cudaStreamSynchronize(h->stream), "upload");   // `chunks` dies here
         }
+    if (h->plan.ring == 4 && m.n_slabs > m.n_kin) {
+        // the ghost slabs as tiles of up to eight consecutive slabs: ufs_dvm_halo_done sums them with the tile kernel's
+        // sums-only pass (a tile's header is all that pass reads)
+        std::vector<TileHdr> gt;
+        for (int64_t s = m.n_kin; s < m.n_slabs; s += TILE_CELLS) {
+            TileHdr t{};
+            t.s0 = (int32_t)s;
+            t.nc = (int32_t)std::min<int64_t>(TILE_CELLS, m.n_slabs - s);
+            gt.push_back(t);
+        }
+        h->n_ghost_tiles = (int64_t)gt.size();
+        if ((rc = upload(h, &h->d_ghost_tiles, gt.data(), gt.size() * sizeof(TileHdr), "upload ghost tiles"))) return rc;
+        CU(cudaStreamSynchronize(h->stream), "upload");   // `gt` dies here
+    }
     h->ghosts_fresh = m.n_slabs == m.n_kin;
     return UFS_DVM_OK;
 }
@@ -402,9 +419,11 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
         }
         CU(launch_step(h->storage, plan, p, h->stream), "step kernel launch");
         h->cur ^= 1;
-        h->parity ^= 1;
+        // every streaming launch draws its tickets from one counter and zeroes the other (the fused exchange has two per step)
+        const int nl = h->plan.ring == 4 ? tiles_launches_per_step(plan, p) : 1;
+        if (nl & 1) h->parity ^= 1;
         if (has_ghosts) h->ghosts_fresh = false;
-        if (h->mesh.n_kin > 0) h->launches += (stream && p.collide) ? 2 : 1;
+        if (h->mesh.n_kin > 0) h->launches += ((stream && p.collide) ? 1 : 0) + nl;
     }
     return UFS_DVM_OK;
 }
@@ -456,7 +475,7 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
         cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
         cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_fluid_pieces);
-        cudaFree(h->d_check); cudaFree(h->d_tile_push);
+        cudaFree(h->d_check); cudaFree(h->d_tile_push); cudaFree(h->d_ghost_tiles);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
@@ -678,10 +697,18 @@ int ufs_dvm_halo_done(ufs_dvm_t h) {
         // the velocity sums of the ghost cells, from the chunks that have just arrived (the step's Maxwellian needs
         // the upwind flux moments of every source; entries of chunks that never arrive are never read)
         StepParams p = make_params(h, 1.0);
-        p.n_kin = (int32_t)n_gh;
-        const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
-        const char* f = static_cast<const char*>(h->f[h->cur]) + (size_t)m.n_kin * m.vel.Nv * elem;
-        CU(launch_sums(h->storage, h->plan, p, f, h->d_sums[h->cur] + (size_t)m.n_kin * SUMS_STRIDE, h->stream), "ghost sums kernel launch");
+        if (h->plan.ring == 4) {
+            // the tile kernel's sums-only pass over the ghost tiles (slab numbers are those of the whole buffer)
+            p.tile_hdr = h->d_ghost_tiles;
+            p.n_tiles = (int32_t)h->n_ghost_tiles;
+            CU(launch_tile_sums(h->storage, h->plan, p, h->f[h->cur], h->d_sums[h->cur], h->stream), "ghost sums kernel launch");
+            h->parity ^= 1;   // the pass drew its tile tickets from this parity's counter and zeroed the other one
+        } else {
+            p.n_kin = (int32_t)n_gh;
+            const size_t elem = h->storage == UFS_STORE_F32 ? 4 : 8;
+            const char* f = static_cast<const char*>(h->f[h->cur]) + (size_t)m.n_kin * m.vel.Nv * elem;
+            CU(launch_sums(h->storage, h->plan, p, f, h->d_sums[h->cur] + (size_t)m.n_kin * SUMS_STRIDE, h->stream), "ghost sums kernel launch");
+        }
         h->launches++;
     }
     h->ghosts_fresh = true;
@@ -709,9 +736,13 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer
     cudaFree(h->d_tile_push);
     h->d_tile_push = nullptr;
     if ((rc = upload(h, &h->d_tile_push, m.tile_push.data(), m.tile_push.size() * sizeof(PushEntry), "upload push entries"))) return rc;
+    // build_push has moved the tiles with push entries to the front: all three tile arrays go up again
     CU(cudaMemcpyAsync(h->d_tile_hdr, m.tiles.data(), m.tiles.size() * sizeof(TileHdr), cudaMemcpyHostToDevice, h->stream), "upload tile headers");
+    CU(cudaMemcpyAsync(h->d_tile_pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4, cudaMemcpyHostToDevice, h->stream), "upload tile piece lists");
+    CU(cudaMemcpyAsync(h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), cudaMemcpyHostToDevice, h->stream), "upload tile index tables");
     CU(cudaStreamSynchronize(h->stream), "upload");
     h->plan.push_on = 1;
+    h->plan.push_tiles = (int32_t)m.n_push_tiles;
     return UFS_DVM_OK;
 }
 

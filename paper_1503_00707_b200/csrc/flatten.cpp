@@ -727,6 +727,31 @@ int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_
             of_slab[s].push_back(e);
         }
     }
+    // tiles with a cell some peer needs come first: k_tiles' PUSH instantiation runs over them, before the plain one runs
+    // over the rest (the pushed rows are on their way while the interior is computed)
+    const size_t nt = m.tiles.size();
+    std::vector<size_t> perm;
+    perm.reserve(nt);
+    auto needed = [&](const TileHdr& t) {
+        for (int c = 0; c < t.nc; c++)
+            if (!of_slab[t.s0 + c].empty()) return true;
+        return false;
+    };
+    for (size_t i = 0; i < nt; i++) if (needed(m.tiles[i])) perm.push_back(i);
+    m.n_push_tiles = (int64_t)perm.size();
+    for (size_t i = 0; i < nt; i++) if (!needed(m.tiles[i])) perm.push_back(i);
+    {
+        const size_t ps = (size_t)8 * m.tile_pmax, cs = (size_t)8 * TILE_CELLS * CELLIDX_BYTES;
+        std::vector<TileHdr> th(nt);
+        std::vector<uint32_t> tp(m.tile_pieces.size());
+        std::vector<uint8_t> tc(m.tile_cellidx.size());
+        for (size_t i = 0; i < nt; i++) {
+            th[i] = m.tiles[perm[i]];
+            std::memcpy(tp.data() + i * ps, m.tile_pieces.data() + perm[i] * ps, ps * 4);
+            std::memcpy(tc.data() + i * cs, m.tile_cellidx.data() + perm[i] * cs, cs);
+        }
+        m.tiles.swap(th); m.tile_pieces.swap(tp); m.tile_cellidx.swap(tc);
+    }
     m.tile_push.clear();
     for (TileHdr& t : m.tiles) {
         t.pad[0] = (int32_t)m.tile_push.size();

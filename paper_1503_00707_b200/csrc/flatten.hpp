@@ -149,6 +149,7 @@ struct FlatMesh {
     std::vector<uint8_t> tile_cellidx;      // [n_tiles][8 octants][TILE_CELLS][CELLIDX_BYTES]
     bool tiles_have_fluid = false;          // some piece is a fluid ghost: the kernel's FLUID instantiation
     std::vector<PushEntry> tile_push;       // fused ghost exchange (build_push): the tiles' push entries
+    int64_t n_push_tiles = 0;               // ... and how many tiles have some (build_push moves them to the front)
 };
 
 // Returns UFS_DVM_OK or an error code with a message in `err`.
@@ -182,7 +183,8 @@ int restrict_to_rank(FlatMesh& m, const int32_t* rank_of_leaf, int my_rank, int 
 // the mesh has them, else runs of consecutive slabs) and fills the tile arrays of `m`.
 void build_tiles(FlatMesh& m, int pmax);
 
-// Fused ghost exchange of a partitioned mesh: fills m.tile_push and the pad words of m.tiles from the send lists.  Per peer
+// Fused ghost exchange of a partitioned mesh: moves the tiles with cells some peer needs to the front of the tile arrays
+// (m.n_push_tiles of them) and fills m.tile_push and the pad words of m.tiles from the send lists.  Per peer
 // rank p: peer_f[b][p] = address (as this device reaches it) of rank p's f buffer b, dest_slab[p][i] = the ghost slab of
 // rank p that takes this rank's i-th send slab (rank p's recv_slab list for this rank), slab_bytes = Nv * element size.
 int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_f1, const int32_t* const* dest_slab, int64_t slab_bytes,

@@ -67,7 +67,8 @@ struct StepLaunch {
     int32_t grid, ncw, pieces, stages;  // ring kernel: CTAs, consumer warps, pieces per octant chunk, ring depth
     cudaEvent_t ev0, ev1;          // if set: recorded on the stream right before / after the main kernel of the step
     int32_t test_stall;            // UFS_DVM_TEST_STALL was set at creation: k_tiles stalls on purpose (watchdog test)
-    int32_t push_on;               // ufs_dvm_halo_push_setup was called: k_tiles also stores the boundary cells into the peers' ghost slabs
+    int32_t push_on;               // ufs_dvm_halo_push_setup was called: the first push_tiles tiles are stepped by k_tiles' PUSH
+    int32_t push_tiles;            //   instantiation (boundary cells also stored into the peers' ghost slabs), then the rest
 };
 
 // per-axis table stride (nodes rounded up to a multiple of 4)
@@ -99,6 +100,7 @@ cudaError_t launch_check_sums(int storage, const StepLaunch& plan, const StepPar
 bool tiles_plan(int storage, const VelLayout& v, int sm_count, StepLaunch* plan, int* pmax);
 void tiles_fluid_pieces(const FlatMesh& m, int storage, std::vector<double>& out);   // host: the table behind StepParams::fluid_pieces
 cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);
+int tiles_launches_per_step(const StepLaunch& plan, const StepParams& p);   // streaming launches of one step (1, or 2 with the fused exchange)
 cudaError_t launch_tile_sums(int storage, const StepLaunch& plan, const StepParams& p, const void* f, double* sums, cudaStream_t stream);
 
 // remap.cu: f of a new mesh from f of the old one (weighted sums of old slabs / frozen fluid Maxwellians)

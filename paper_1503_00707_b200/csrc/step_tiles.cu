@@ -321,13 +321,19 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
             }
         }
         T* const gcell = reinterpret_cast<T*>(p.f_out) + (int64_t)(s0 + c) * p.Nv;
-        // fused ghost exchange: the push entries of this thread's cell (flatten.hpp: PushEntry)
-        int pfirst = 0, pcnt = 0;
+        // fused ghost exchange: the push entries of this thread's cell (flatten.hpp: PushEntry).  pinfo bits 0..7: the octants
+        // some peer needs, bits 8..11: entries; a cell nobody needs (almost all of them) costs one predicate per store
+        int pfirst = 0;
+        uint32_t pinfo = 0u;
         if constexpr (PUSH) {
             const uint32_t cnts = *reinterpret_cast<const uint32_t*>(smem_raw + hdr + 28);
-            pfirst = *reinterpret_cast<const int*>(smem_raw + hdr + 24);
-            for (int i = 0; i < c; i++) pfirst += (int)((cnts >> (4 * i)) & 15u);
-            pcnt = active ? (int)((cnts >> (4 * c)) & 15u) : 0;
+            if (cnts != 0u && active) {
+                pfirst = *reinterpret_cast<const int*>(smem_raw + hdr + 24);
+                for (int i = 0; i < c; i++) pfirst += (int)((cnts >> (4 * i)) & 15u);
+                const uint32_t pcnt = (cnts >> (4 * c)) & 15u;
+                for (uint32_t e = 0; e < pcnt; e++) pinfo |= __ldg(&p.tile_push[pfirst + e].info) & 0xffu;
+                pinfo |= pcnt << 8;
+            }
         }
         double* const red = reinterpret_cast<double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)(c * 3 + gi) * SUMS_STRIDE;
         for (int q = 0; q < NQ; q++) {
@@ -397,23 +403,34 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                     const uint32_t flags = (ix.x >> 8) & 0xffu;
                     T* const gdst = gcell + (int64_t)o * CH + (int64_t)row * THX + k0;
                     // the peers' ghost slabs that take this cell's chunk of octant o: the same row goes there as well
-                    T* pd[PUSH ? PUSH_PER_CELL_MAX : 1];
-                    if constexpr (PUSH) {
-#pragma unroll
-                        for (int e = 0; e < PUSH_PER_CELL_MAX; e++) {
-                            pd[e] = nullptr;
-                            if (e < pcnt) {
-                                const PushEntry* ent = p.tile_push + pfirst + e;
-                                if ((__ldg(&ent->info) >> o) & 1u)
-                                    pd[e] = reinterpret_cast<T*>(__ldg(reinterpret_cast<const unsigned long long*>(ent->dst) + p.push_parity)) + ((int64_t)o * CH + (int64_t)row * THX + k0);
-                            }
-                        }
-                    }
+                    const bool po = PUSH && ((pinfo >> o) & 1u);
                     auto push_out = [&](int j, const T (&out)[VEC]) {
                         if constexpr (PUSH) {
+                            if (po) {
+                                const int pc = (int)(pinfo >> 8);
+                                for (int e = 0; e < pc; e++) {
+                                    const PushEntry* ent = p.tile_push + pfirst + e;
+                                    if ((__ldg(&ent->info) >> o) & 1u)
+                                        stg16(reinterpret_cast<T*>(__ldg(reinterpret_cast<const unsigned long long*>(ent->dst) + p.push_parity))
+                                                  + (gdst - gcell) + j * VEC, out);
+                                }
+                            }
+                        }
+                    };
+                    // unrolled row loops keep the row's vectors and push once, after the loop (one cold block per loop)
+                    T outs[PUSH ? RV : 1][VEC];
+                    auto keep_out = [&](int j, const T (&out)[VEC]) {
+                        if constexpr (PUSH) {
 #pragma unroll
-                            for (int e = 0; e < PUSH_PER_CELL_MAX; e++)
-                                if (pd[e]) stg16(pd[e] + j * VEC, out);
+                            for (int i = 0; i < VEC; i++) outs[j][i] = out[i];
+                        }
+                    };
+                    auto push_row = [&]() {
+                        if constexpr (PUSH) {
+                            if (po) {
+#pragma unroll
+                                for (int j = 0; j < RV; j++) push_out(j, outs[j]);
+                            }
                         }
                     };
                     T wb = T(0);
@@ -472,12 +489,13 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 }
                             }
                             stg16_cs(gdst + j * VEC, out);
-                            push_out(j, out);
+                            keep_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 row_sums((double)out[i], j * VEC + i);
                             }
                         }
+                        push_row();
                     } else if (FLUID && (flags & CIDX_FOUR) == 0u) {
                         // one source per axis, some of them fluid leaves (the common cell under a kinetic/fluid mask): a
                         // piece is read, a fluid source is row factor x x factor from its mini-piece (flatten.hpp)
@@ -518,12 +536,13 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 for (int i = 0; i < VEC; i++) out[i] += wb * gx[i];
                             }
                             stg16_cs(gdst + j * VEC, out);
-                            push_out(j, out);
+                            keep_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 row_sums((double)out[i], j * VEC + i);
                             }
                         }
+                        push_row();
                     } else {
                         // 2:1 faces towards finer leaves (four sources, each weighted 1/4: reading G3) and / or fluid leaves
                         const uint32_t words[3] = {ix.y, ix.z, ix.w};
@@ -587,12 +606,13 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                                 }
                             }
                             stg16_cs(gdst + j * VEC, out);
-                            push_out(j, out);
+                            if constexpr (FLUID) push_out(j, out); else keep_out(j, out);
 #pragma unroll
                             for (int i = 0; i < VEC; i++) {
                                 if constexpr (FLUID) row_sums_dyn((double)out[i], j * VEC + i); else row_sums((double)out[i], j * VEC + i);
                             }
                         }
+                        if constexpr (!FLUID) push_row();
                     }
                 }
                 __syncwarp();
@@ -744,14 +764,43 @@ cudaError_t launch_tiles(int storage, const StepLaunch& plan, const StepParams& 
     cudaError_t e = launch_prep(storage, p, st);
     if (e != cudaSuccess) return e;
     if (plan.push_on) {
-        // fused ghost exchange: the same pass, boundary cells stored a second time into the peers' ghost slabs
+        // fused ghost exchange: first the tiles with cells some peer needs (their rows are also stored into the peers' ghost
+        // slabs and travel while the rest is computed), then the plain pass over the other tiles.  Two launches, two ticket
+        // counters: each launch draws from one and zeroes the other.
+        const int nb = plan.push_tiles < p.n_tiles ? plan.push_tiles : p.n_tiles;
+        StepLaunch pl = plan;
+        cudaEvent_t ev1 = plan.ev1;
+        if (nb > 0) {
+            StepParams q = p;
+            q.n_tiles = nb;
+            if (nb < p.n_tiles) pl.ev1 = nullptr;
+            if (storage == UFS_STORE_F32)
+                e = p.tiles_have_fluid ? launch_tiles_t<float, true, false, true>(pl, q, st, true) : launch_tiles_t<float, false, false, true>(pl, q, st, true);
+            else
+                e = p.tiles_have_fluid ? launch_tiles_t<double, true, false, true>(pl, q, st, true) : launch_tiles_t<double, false, false, true>(pl, q, st, true);
+            if (e != cudaSuccess || nb == p.n_tiles) return e;
+            pl.ev0 = nullptr;
+        }
+        StepParams q = p;
+        q.n_tiles = p.n_tiles - nb;
+        q.tile_hdr = p.tile_hdr + nb;
+        q.tile_pieces = p.tile_pieces + (size_t)nb * 8 * p.tile_pmax;
+        q.tile_cellidx = p.tile_cellidx + (size_t)nb * 8 * TILE_CELLS * CELLIDX_BYTES;
+        if (nb > 0) { q.counter = p.counter_reset; q.counter_reset = p.counter; }
+        pl.ev1 = ev1;
         if (storage == UFS_STORE_F32)
-            return p.tiles_have_fluid ? launch_tiles_t<float, true, false, true>(plan, p, st, true) : launch_tiles_t<float, false, false, true>(plan, p, st, true);
-        return p.tiles_have_fluid ? launch_tiles_t<double, true, false, true>(plan, p, st, true) : launch_tiles_t<double, false, false, true>(plan, p, st, true);
+            return p.tiles_have_fluid ? launch_tiles_t<float, true, false>(pl, q, st, true) : launch_tiles_t<float, false, false>(pl, q, st, true);
+        return p.tiles_have_fluid ? launch_tiles_t<double, true, false>(pl, q, st, true) : launch_tiles_t<double, false, false>(pl, q, st, true);
     }
     if (storage == UFS_STORE_F32)
         return p.tiles_have_fluid ? launch_tiles_t<float, true, false>(plan, p, st, true) : launch_tiles_t<float, false, false>(plan, p, st, true);
     return p.tiles_have_fluid ? launch_tiles_t<double, true, false>(plan, p, st, true) : launch_tiles_t<double, false, false>(plan, p, st, true);
+}
+
+int tiles_launches_per_step(const StepLaunch& plan, const StepParams& p) {
+    if (!plan.push_on) return 1;
+    const int nb = plan.push_tiles < p.n_tiles ? plan.push_tiles : p.n_tiles;
+    return (nb > 0 ? 1 : 0) + (nb < p.n_tiles ? 1 : 0);
 }
 
 // sums[n_kin][SUMS_STRIDE] of an f the caller has just written: the same kernel, own chunks only, no store

@@ -38,7 +38,7 @@ def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False):
             for _ in range(nsteps):
                 step_pushed_local(ranks, case.dt)
             for r, b in zip(ranks, before):
-                per_step = 2 + (1 if r.n_ghost else 0)         # k_prep, k_tiles, ghost sums
+                per_step = 3 + (1 if r.n_ghost else 0)         # k_prep, k_tiles on the boundary tiles, on the rest, ghost sums
                 first = 1 if r.n_inner else 0                  # the sums pass of the initial f
                 assert B.ufs_dvm_launch_count(r.h) - b <= nsteps * per_step + first
         else:
@@ -112,11 +112,13 @@ def test_step_without_fresh_ghosts_is_refused():
             r.close()
 
 
-def test_partitioned_config3_at_stated_size_four_ranks():
+@pytest.mark.parametrize("push", [False, True])
+def test_partitioned_config3_at_stated_size_four_ranks(push):
     """Config 3 literal (26 312 leaves: inflow, outflow, specular sides, SOLID body, 2:1 faces) cut into four ranks on one
-    device, 5 steps with the ghost exchange before each; the stitched whole field against the one-domain oracle."""
+    device, 5 steps with the ghost exchange before each (packed, or fused into the step kernel); the stitched whole field
+    against the one-domain oracle."""
     case = inputs.config3(lmax=7)
-    f0, f, mom, sent = _run_partitioned(case, 4, 5)
+    f0, f, mom, sent = _run_partitioned(case, 4, 5, push=push)
     assert sent > 0
     o = Oracle(case)
     f_ref = o.step(f0, case.dt, 5)
@@ -162,6 +164,14 @@ def test_fused_exchange_push_entries_cover_the_send_lists():
             assert np.all(counts[np.arange(8)[None, :] >= t["nc"][:, None]] == 0)
             n_send = sum(B.ufs_dvm_halo(r.h, p)["send_slab"].size for p in range(3))
             assert counts.sum() == n_send
+            # the tiles with entries come first (they are stepped first, by the pushing instantiation)
+            has = counts.sum(axis=1) > 0
+            assert 0 < has.sum() < t["n_tiles"] and np.all(has[:has.sum()]) and not np.any(has[has.sum():])
+            # every inner slab is in exactly one tile, whatever the order
+            cover = np.zeros(r.n_inner, np.int64)
+            for i in range(t["n_tiles"]):
+                cover[t["s0"][i]:t["s0"][i] + t["nc"][i]] += 1
+            assert np.all(cover == 1)
             # a tile's entries follow the previous tile's
             assert np.array_equal(t["push_first"], np.concatenate([[0], np.cumsum(counts.sum(axis=1))[:-1]]))
             # per cell: as many entries as peers that list it
