@@ -255,6 +255,13 @@ int ufs_dvm_halo_done(ufs_dvm_t h);
  * more than four peers (then the pack / unpack exchange serves).  May be called again (new peer addresses). */
 int ufs_dvm_halo_push_setup(ufs_dvm_t h, void *const *peer_f0, void *const *peer_f1, const int32_t *const *dest_slab);
 
+/* The push entries that ufs_dvm_halo_push_setup built (it also accepts a host-only handle: the records are built, nothing
+ * is uploaded; the addresses are then just numbers), in the order the kernel reads them (HOST outputs, any may be NULL):
+ * *n_entries, *n_push_tiles (the tiles with entries: the first ones of ufs_dvm_tiles); per entry: slab = the inner slab whose
+ * rows are pushed, mask = the octants pushed, dst0 / dst1 = address of the peer's ghost slab in its f buffer 0 / 1. */
+int ufs_dvm_push_entries(ufs_dvm_t h, int64_t *n_entries, int64_t *n_push_tiles, int32_t *slab, uint8_t *mask, uint64_t *dst0,
+                         uint64_t *dst1);
+
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),
  * level per cell (8 bytes), first push entry, eight 4-bit push counts (0, 0 without ufs_dvm_halo_push_setup)}; pieces[n_tiles][8][pmax] = source chunk codes: bits 0..29 = index * 8 + octant, the

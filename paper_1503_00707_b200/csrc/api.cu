@@ -717,7 +717,6 @@ int ufs_dvm_halo_done(ufs_dvm_t h) {
 
 int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer_f1, const int32_t* const* dest_slab) {
     if (!h) return UFS_DVM_EINVAL;
-    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (h->sticky) return h->sticky;
     if (!h->mesh.partial) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh");
     if (h->plan.ring != 4) return fail(h, UFS_DVM_EINVAL, "the fused ghost exchange needs the tile kernel (k_tiles)");
@@ -732,6 +731,9 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer
         return fail(h, UFS_DVM_ENOMEM, "out of host memory");
     }
     if (rc) return fail(h, rc, err);
+    h->plan.push_on = 1;
+    h->plan.push_tiles = (int32_t)m.n_push_tiles;
+    if (!h->device) return UFS_DVM_OK;   // host-only handle: the records are built (ufs_dvm_push_entries), nothing to upload
     CU(cudaStreamSynchronize(h->stream), "stream synchronize");   // no step in flight reads the old headers
     cudaFree(h->d_tile_push);
     h->d_tile_push = nullptr;
@@ -741,8 +743,25 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer
     CU(cudaMemcpyAsync(h->d_tile_pieces, m.tile_pieces.data(), m.tile_pieces.size() * 4, cudaMemcpyHostToDevice, h->stream), "upload tile piece lists");
     CU(cudaMemcpyAsync(h->d_tile_cellidx, m.tile_cellidx.data(), m.tile_cellidx.size(), cudaMemcpyHostToDevice, h->stream), "upload tile index tables");
     CU(cudaStreamSynchronize(h->stream), "upload");
-    h->plan.push_on = 1;
-    h->plan.push_tiles = (int32_t)m.n_push_tiles;
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_push_entries(ufs_dvm_t h, int64_t* n_entries, int64_t* n_push_tiles, int32_t* slab, uint8_t* mask, uint64_t* dst0, uint64_t* dst1) {
+    if (!h) return UFS_DVM_EINVAL;
+    const FlatMesh& m = h->mesh;
+    if (!h->plan.push_on) return fail(h, UFS_DVM_EINVAL, "ufs_dvm_halo_push_setup has not been called");
+    if (n_entries) *n_entries = (int64_t)m.tile_push.size();
+    if (n_push_tiles) *n_push_tiles = m.n_push_tiles;
+    for (const TileHdr& t : m.tiles) {
+        int64_t e = t.pad[0];
+        for (int c = 0; c < t.nc; c++)
+            for (uint32_t k = 0; k < (((uint32_t)t.pad[1] >> (4 * c)) & 15u); k++, e++) {
+                if (slab) slab[e] = t.s0 + c;
+                if (mask) mask[e] = (uint8_t)(m.tile_push[e].info & 0xffu);
+                if (dst0) dst0[e] = m.tile_push[e].dst[0];
+                if (dst1) dst1[e] = m.tile_push[e].dst[1];
+            }
+    }
     return UFS_DVM_OK;
 }
 

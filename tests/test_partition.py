@@ -148,6 +148,52 @@ def test_one_face_ghost_gets_only_its_four_upwind_chunks():
     B.ufs_dvm_destroy(h)
 
 
+@pytest.mark.parametrize("name,n_ranks", [("small3_walls_solid", 2), ("small3_walls_solid", 5), ("small5_mask", 3)])
+def test_push_entries_pair_every_send_slab_with_the_peers_ghost_slab(name, n_ranks):
+    """ufs_dvm_halo_push_setup on host-only handles (made-up buffer addresses): one entry per (sent cell, peer) with the
+    send list's octant mask and the address of the ghost slab the PEER's receive list names for it, in both f buffers; the
+    tiles with entries first."""
+    case = _cases()[name]
+    desc, keep = B.make_desc(case)
+    rol = B.ufs_dvm_partition(desc, n_ranks)
+    hs = [B.ufs_dvm_create_part_host(desc, rol, r, n_ranks) for r in range(n_ranks)]
+    slab_bytes = case.Nv * 8
+    base = lambda p, b: 4096 * (1 + 2 * p + b) * (1 << 32)
+    try:
+        for r in range(n_ranks):
+            with pytest.raises(B.UfsDvmError):
+                B.ufs_dvm_push_entries(hs[r])                       # not set up yet
+            dest = [None if p == r else B.ufs_dvm_halo(hs[p], r)["recv_slab"] for p in range(n_ranks)]
+            B.ufs_dvm_halo_push_setup(hs[r], [None if p == r else base(p, 0) for p in range(n_ranks)],
+                                      [None if p == r else base(p, 1) for p in range(n_ranks)], dest)
+            ent = B.ufs_dvm_push_entries(hs[r])
+            want = set()
+            for p in range(n_ranks):
+                if p == r:
+                    continue
+                hl = B.ufs_dvm_halo(hs[r], p)
+                for s, m, d in zip(hl["send_slab"], hl["send_mask"], dest[p]):
+                    want.add((int(s), int(m), base(p, 0) + int(d) * slab_bytes, base(p, 1) + int(d) * slab_bytes))
+            got = list(zip(ent["slab"].tolist(), ent["mask"].tolist(), ent["dst0"].tolist(), ent["dst1"].tolist()))
+            assert len(got) == len(set(got)) and set(got) == want
+            t = B.ufs_dvm_tiles(hs[r])
+            sent = np.zeros(B.ufs_dvm_part_layout(hs[r])["n_inner"], bool)
+            sent[ent["slab"]] = True
+            has = np.array([sent[t["s0"][i]:t["s0"][i] + t["nc"][i]].any() for i in range(t["n_tiles"])])
+            assert ent["n_push_tiles"] == has.sum() and np.all(has[:has.sum()]) and not np.any(has[has.sum():])
+            # inside each group the tiles keep their N-order
+            for grp in (t["s0"][:has.sum()], t["s0"][has.sum():]):
+                assert np.all(np.diff(grp) > 0)
+            # a second set-up with the same arguments changes nothing
+            B.ufs_dvm_halo_push_setup(hs[r], [None if p == r else base(p, 0) for p in range(n_ranks)],
+                                      [None if p == r else base(p, 1) for p in range(n_ranks)], dest)
+            ent2 = B.ufs_dvm_push_entries(hs[r])
+            assert all(np.array_equal(ent[k], ent2[k]) for k in ("slab", "mask", "dst0", "dst1"))
+    finally:
+        for h in hs:
+            B.ufs_dvm_destroy(h)
+
+
 # ----------------------------------------------------------------------------------------------- two ranks, gloo
 def _free_port():
     with socket.socket() as s:
@@ -162,7 +208,7 @@ def _octant_of_velocity(case):
     return ((kx >= nv[0] // 2) * 1 + (ky >= nv[1] // 2) * 2 + (kz >= nv[2] // 2) * 4).ravel()
 
 
-def _rank_worker(rank, world, port, which, nsteps, out):
+def _rank_worker(rank, world, port, which, nsteps, out, fused=False):
     import torch
     import torch.distributed as dist
     from oracle.dvm_oracle import Oracle
@@ -193,6 +239,28 @@ def _rank_worker(rank, world, port, which, nsteps, out):
     f[ghost_rows] *= 0.37                                         # garbage until the exchange fills what is needed
     octv = _octant_of_velocity(case)
     halos = {p: B.ufs_dvm_halo(h, p) for p in range(world) if p != rank}
+    if fused:
+        # fused exchange (ufs_dvm_halo_push_setup on the host-only handle): what travels, and WHERE it lands in the peer, comes
+        # from this rank's push entries -- made-up buffer addresses, decoded back to (peer, ghost slab) -- not from the
+        # peer's own receive list.  The peers' receive lists are the set-up input, exchanged once.
+        recv_lists = [None] * world
+        dist.all_gather_object(recv_lists, {p: hl["recv_slab"] for p, hl in halos.items()})
+        slab_bytes = case.Nv * 8
+        base = lambda p, b: ((p + 1) << 44) + (b << 43)
+        B.ufs_dvm_halo_push_setup(h, [None if p == rank else base(p, 0) for p in range(world)],
+                                  [None if p == rank else base(p, 1) for p in range(world)],
+                                  [None if p == rank else recv_lists[p][rank] for p in range(world)])
+        ent = B.ufs_dvm_push_entries(h)
+        assert np.all(ent["dst1"] - ent["dst0"] == (1 << 43))
+        peer_of = (ent["dst0"] >> np.uint64(44)).astype(np.int64) - 1
+        dest_of = ((ent["dst0"] & np.uint64((1 << 43) - 1)) // np.uint64(slab_bytes)).astype(np.int64)
+        assert np.all((ent["dst0"] & np.uint64((1 << 43) - 1)) % np.uint64(slab_bytes) == 0)
+        for p, hl in halos.items():
+            mine = np.nonzero(peer_of == p)[0]
+            mine = mine[np.argsort(dest_of[mine], kind="stable")]
+            # the same chunks as the send list, each with the ghost slab the peer expects it in
+            assert sorted(zip(ent["slab"][mine].tolist(), ent["mask"][mine].tolist())) == sorted(zip(hl["send_slab"].tolist(), hl["send_mask"].tolist()))
+            halos[p] = dict(hl, send_slab=ent["slab"][mine], send_mask=ent["mask"][mine], send_dest=dest_of[mine])
     for _ in range(nsteps):
         reqs, recv = [], {}
         for p, hl in halos.items():
@@ -203,9 +271,21 @@ def _rank_worker(rank, world, port, which, nsteps, out):
             reqs += [dist.isend(send, p), dist.irecv(recv[p], p)]
         for q in reqs:
             q.wait()
+        dests = {}
+        if fused:      # the senders' destinations travel with the data: the receiver places every chunk where it was pushed
+            for p, hl in halos.items():
+                theirs = torch.empty(len(hl["recv_slab"]), dtype=torch.int64)
+                rq = [dist.isend(torch.from_numpy(np.ascontiguousarray(hl["send_dest"], np.int64)), p), dist.irecv(theirs, p)]
+                for q in rq:
+                    q.wait()
+                dests[p] = theirs.numpy()
         for p, hl in halos.items():
             buf, at = recv[p].numpy(), 0
-            for s, m in zip(hl["recv_slab"], hl["recv_mask"]):
+            where = dests[p] if fused else hl["recv_slab"]
+            assert sorted(where.tolist()) == sorted(hl["recv_slab"].tolist())
+            mask_of = {int(s): int(m) for s, m in zip(hl["recv_slab"], hl["recv_mask"])}
+            for s in where:
+                m = mask_of[int(s)]
                 sel = (int(m) >> octv) & 1 == 1
                 k = int(sel.sum())
                 f[row[int(slabs[s])], sel] = buf[at:at + k]
@@ -219,13 +299,14 @@ def _rank_worker(rank, world, port, which, nsteps, out):
     B.ufs_dvm_destroy(h)
 
 
-@pytest.mark.parametrize("which,nsteps", [("random_periodic", 4), ("small3_walls_solid", 2)])
-def test_two_rank_gloo_run_stitched_equals_the_one_domain_oracle(which, nsteps):
+@pytest.mark.parametrize("which,nsteps,fused", [("random_periodic", 4, False), ("small3_walls_solid", 2, False),
+                                                ("small3_walls_solid", 2, True)])
+def test_two_rank_gloo_run_stitched_equals_the_one_domain_oracle(which, nsteps, fused):
     from oracle.dvm_oracle import Oracle
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_rank_worker, args=(r, 2, port, which, nsteps, out)) for r in range(2)]
+    procs = [ctx.Process(target=_rank_worker, args=(r, 2, port, which, nsteps, out, fused)) for r in range(2)]
     for p in procs:
         p.start()
     got = [out.get(timeout=600) for _ in range(2)]
