@@ -181,3 +181,92 @@ def test_config4_lit_windows_and_conservation():
     """The literal 32-box tree (about 4.5e5 leaves)."""
     case = inputs.config4(target_leaves=None)
     _windowed_parity_and_conservation(case, case.nsteps)
+
+
+# ------------------------------------------------------------------------------------ config 4 cut into eight ranks
+def test_config4_eight_ranks_fused_exchange_windows_and_conservation():
+    """bench.py --emulate-ranks 8 --fused-exchange at the stated size: config 4 cut into eight ranks on one device, the
+    ghost cells written by the peers' step kernels (ufs_dvm_halo_push_setup).  Windowed oracle (S = 3) at cells the
+    exchange touches -- cells a rank sends, drawn from every rank's send lists, whose windows reach across the cut -- and at
+    random inner cells; totals conserved over the config's 10 steps, summed over the ranks."""
+    import torch
+    from paper_1503_00707_b200.partition import RankStepper, exchange_local, setup_push_local, step_pushed_local
+    case = inputs.config4()
+    n_ranks = 8
+    free, _ = torch.cuda.mem_get_info()
+    assert free >= 1.2 * 2 * case.n_leaves * case.Nv * 4 + (4 << 30), "needs about 140 GiB of device memory"
+    desc, keep = B.make_desc(case)
+    rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, 0.0)
+    ranks = [RankStepper(case, rol, r, n_ranks) for r in range(n_ranks)]
+    try:
+        rng = np.random.default_rng(inputs.SEED_BASE + 408)
+        owner = np.full(case.n_leaves, -1, np.int64)
+        local = np.full(case.n_leaves, -1, np.int64)
+        centres = []
+        for r in ranks:
+            assert B.ufs_dvm_kernel_name(r.h) == STEP_KERNEL
+            harness.fill_initial_f_device(r, case)
+            owner[r.cell_of_slab] = r.my_rank
+            local[r.cell_of_slab] = np.arange(r.n_inner)
+            sent = np.unique(np.concatenate([B.ufs_dvm_halo(r.h, p)["send_slab"] for p in r.peers]))
+            assert sent.size > 0
+            centres.append(r.cell_of_slab[rng.choice(sent, 8, replace=False)])
+            centres.append(r.cell_of_slab[rng.choice(r.n_inner, 3, replace=False)])
+        centres = np.unique(np.concatenate(centres))
+        kin = np.nonzero(case.kind == inputs.CELL_KINETIC)[0]
+        assert np.all(owner[kin] >= 0)
+
+        def read_leaves(leaves):
+            out = np.empty((leaves.size, case.Nv))
+            for r in ranks:
+                sel = np.nonzero(owner[leaves] == r.my_rank)[0]
+                if sel.size:
+                    out[sel] = r.read_canonical(local[leaves[sel]])
+            return out
+
+        def totals():
+            tot = np.zeros(5)
+            for r in ranks:
+                m = r.moments()                                       # rows: the rank's leaves in ascending leaf order
+                tot += (m * 8.0 ** (-case.level[r.inner_leaves].astype(np.float64))).sum(axis=1)
+            return tot
+
+        mesh = Oracle(case)
+        windows = []
+        for c in centres.tolist():
+            ids = harness.window_leaves(case, c, S_WIN, mesh.leaf_neighbours)
+            kin_ids = ids[case.kind[ids] == inputs.CELL_KINETIC]
+            windows.append((c, ids, kin_ids, read_leaves(kin_ids)))
+        del mesh
+        # every sampled send cell's window holds cells of another rank
+        assert sum(np.unique(owner[w[2]]).size > 1 for w in windows) >= 8 * n_ranks // 2
+        setup_push_local(ranks)
+        exchange_local(ranks)                                         # the ghosts of the first step
+        tot0 = totals()
+        for _ in range(S_WIN):
+            step_pushed_local(ranks, case.dt)
+        f_c = read_leaves(centres)
+        worst = 0.0
+        for n, (c, ids, kin_ids, f0) in enumerate(windows):
+            o = Oracle(harness.sub_case(case, ids), window=True)
+            f_ref = o.step(f0, case.dt, S_WIN)
+            k = int(np.searchsorted(kin_ids, c))
+            err = np.abs(f_c[n] - f_ref[k]).max() / np.abs(f_ref[k]).max()
+            worst = max(worst, err)
+            assert err <= TOL_F32, f"leaf {c} (rank {owner[c]}, level {case.level[c]}): f {err:.3e}"
+        print(f"config 4 in {n_ranks} ranks, fused exchange: {len(windows)} windows "
+              f"({sum(np.unique(owner[w[2]]).size > 1 for w in windows)} across a cut), "
+              f"{sum(r.n_inner for r in ranks)} inner + {sum(r.n_ghost for r in ranks)} ghost cells, worst f error {worst:.2e}")
+        for _ in range(case.nsteps - S_WIN):
+            step_pushed_local(ranks, case.dt)
+        tot1 = totals()
+        scale = np.array([tot0[0], max(np.abs(tot0[1:4]).max(), 0.1 * tot0[0]), 0, 0, tot0[4]])
+        scale[2] = scale[3] = scale[1]
+        drift = np.abs(tot1 - tot0) / scale
+        assert drift.max() <= 1e-8, f"totals drift {drift} over {case.nsteps} steps in {n_ranks} ranks"
+    finally:
+        for r in ranks:
+            r.close()
+            r.f = None
+        gc.collect()
+        torch.cuda.empty_cache()
