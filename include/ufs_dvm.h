@@ -223,17 +223,21 @@ int ufs_dvm_part_layout(ufs_dvm_t h, int64_t *n_inner, int64_t *n_ghost, int64_t
 int ufs_dvm_halo(ufs_dvm_t h, int32_t peer, int64_t *n_send, int32_t *send_slab, uint8_t *send_mask,
                  int64_t *n_recv, int32_t *recv_slab, uint8_t *recv_mask);
 
-/* Sizes in bytes of the packed buffers exchanged with `peer` (HOST outputs): listed chunks x chunk size. */
+/* Sizes in bytes of the packed buffers exchanged with `peer` (HOST outputs): listed chunks x chunk size, then 36 doubles per
+ * listed cell (its carried velocity sums; none with the one-CTA-per-cell kernels, which carry no sums). */
 int ufs_dvm_halo_bytes(ufs_dvm_t h, int32_t peer, int64_t *send_bytes, int64_t *recv_bytes);
 
 /* Enqueue: gather the chunks of the send list of `peer` from the current f into buf_dev (DEVICE, 16-byte aligned,
- * send_bytes), entries in list order, a slab's chunks by ascending octant / scatter buf_dev (recv_bytes) into the ghost
- * slabs of the current f. */
+ * send_bytes), entries in list order, a slab's chunks by ascending octant, and behind them the listed cells' carried sums
+ * (formed first if f has not been summed yet) / scatter buf_dev (recv_bytes) into the ghost slabs of the current f and the
+ * ghost rows of its sums.  The ghost rows thus hold the OWNER's sums, and a partitioned run is bit-identical to the
+ * one-domain run. */
 int ufs_dvm_halo_pack(ufs_dvm_t h, int32_t peer, void *buf_dev);
 int ufs_dvm_halo_unpack(ufs_dvm_t h, int32_t peer, const void *buf_dev);
 
-/* Every peer's chunks have been unpacked (enqueued on the handle's stream): enqueue the velocity sums of the ghost cells
- * and allow the next ufs_dvm_step. */
+/* Every peer's chunks have been unpacked (enqueued on the handle's stream), or pushed by the peers' step kernels (below):
+ * allow the next ufs_dvm_step.  Where the ghost cells' sums did not arrive with their f (fused exchange set up without
+ * peer_sums) they are formed here from the ghost slabs, one pass of the sums kernel over them. */
 int ufs_dvm_halo_done(ufs_dvm_t h);
 
 /* Fused ghost exchange: step and exchange in ONE kernel over peer memory (PAPER.md:185-187 does the exchange as separate
@@ -251,16 +255,28 @@ int ufs_dvm_halo_done(ufs_dvm_t h);
  * then on, per step:  ufs_dvm_step(h, dt, 1) on every rank  ->  a barrier ACROSS the ranks' streams (every rank's step kernel
  * has finished: its ghost slabs are complete, and nobody still reads the buffers the next step will push into)  ->
  * ufs_dvm_halo_done(h) (ghost sums)  ->  next step.  Double buffering makes that one barrier per step enough.
+ * peer_sums0 / peer_sums1 (both or neither; arrays of n_ranks entries like peer_f0): rank p's two arrays of carried velocity
+ * sums (ufs_dvm_sums_dev on rank p).  With them the step kernel also writes the 36 sums of every pushed cell into the
+ * peer's ghost row, ufs_dvm_halo_done has no pass over the ghost slabs left to launch, and -- the ghost rows now holding the
+ * owner's own carried sums, not a re-summation -- the partitioned run is bit-identical to the one-domain run.  Every rank
+ * must then be set up the same way.  NULL: ufs_dvm_halo_done sums the ghost slabs as after an ordinary exchange.
  * EINVAL: not a partitioned handle, not the tile kernel, a needed entry is NULL or misaligned, or some cell is needed by
  * more than four peers (then the pack / unpack exchange serves).  May be called again (new peer addresses). */
-int ufs_dvm_halo_push_setup(ufs_dvm_t h, void *const *peer_f0, void *const *peer_f1, const int32_t *const *dest_slab);
+int ufs_dvm_halo_push_setup(ufs_dvm_t h, void *const *peer_f0, void *const *peer_f1, const int32_t *const *dest_slab,
+                            void *const *peer_sums0, void *const *peer_sums1);
+
+/* DEVICE addresses of the handle's two arrays of carried velocity sums ([n_inner + n_ghost][36] doubles, library-owned,
+ * valid until ufs_dvm_destroy): what a peer passes as peer_sums0 / peer_sums1 above (the same process: the pointers
+ * themselves with peer access enabled; another process: their cudaIpcOpenMemHandle mappings). */
+int ufs_dvm_sums_dev(ufs_dvm_t h, void **sums0, void **sums1);
 
 /* The push entries that ufs_dvm_halo_push_setup built (it also accepts a host-only handle: the records are built, nothing
  * is uploaded; the addresses are then just numbers), in the order the kernel reads them (HOST outputs, any may be NULL):
  * *n_entries, *n_push_tiles (the tiles with entries: the first ones of ufs_dvm_tiles); per entry: slab = the inner slab whose
- * rows are pushed, mask = the octants pushed, dst0 / dst1 = address of the peer's ghost slab in its f buffer 0 / 1. */
+ * rows are pushed, mask = the octants pushed, dst0 / dst1 = address of the peer's ghost slab in its f buffer 0 / 1,
+ * sums0 / sums1 = address of that ghost cell's row in the peer's sums array 0 / 1 (0 if the sums are not pushed). */
 int ufs_dvm_push_entries(ufs_dvm_t h, int64_t *n_entries, int64_t *n_push_tiles, int32_t *slab, uint8_t *mask, uint64_t *dst0,
-                         uint64_t *dst1);
+                         uint64_t *dst1, uint64_t *sums0, uint64_t *sums1);
 
 /* The tile records the flattener built for k_tiles (HOST outputs, any may be NULL; all empty for other kernels):
  * *n_tiles, *pmax (stride of the piece lists); hdr[n_tiles][8] int32 = {first slab, cells, pieces per octant (8 bytes),

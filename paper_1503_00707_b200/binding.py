@@ -23,7 +23,7 @@ EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_mom
            "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan",
            "ufs_dvm_partition", "ufs_dvm_create_part", "ufs_dvm_create_part_host", "ufs_dvm_part_layout", "ufs_dvm_halo",
            "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done", "ufs_dvm_moments_static",
-           "ufs_dvm_halo_push_setup", "ufs_dvm_push_entries"]
+           "ufs_dvm_halo_push_setup", "ufs_dvm_push_entries", "ufs_dvm_sums_dev"]
 
 STATIC_MAX_CELLS = 8192   # UFS_DVM_STATIC_MAX_CELLS of include/ufs_dvm.h
 
@@ -79,8 +79,9 @@ def lib() -> C.CDLL:
         L.ufs_dvm_halo_pack.argtypes = [vp, C.c_int32, vp]
         L.ufs_dvm_halo_unpack.argtypes = [vp, C.c_int32, vp]
         L.ufs_dvm_halo_done.argtypes = [vp]
-        L.ufs_dvm_halo_push_setup.argtypes = [vp, vp, vp, vp]
-        L.ufs_dvm_push_entries.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp, vp, vp, vp]
+        L.ufs_dvm_halo_push_setup.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.ufs_dvm_sums_dev.argtypes = [vp, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]
+        L.ufs_dvm_push_entries.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.ufs_dvm_last_error.argtypes = [vp]; L.ufs_dvm_last_error.restype = C.c_char_p
@@ -300,24 +301,31 @@ def ufs_dvm_halo_done(h):
     _check(h, lib().ufs_dvm_halo_done(h))
 
 
-def ufs_dvm_halo_push_setup(h, peer_f0, peer_f1, dest_slab):
+def ufs_dvm_halo_push_setup(h, peer_f0, peer_f1, dest_slab, peer_sums0=None, peer_sums1=None):
     """peer_f0 / peer_f1: per rank the device address of that rank's f buffers (None for ranks that need nothing from this
-    one); dest_slab: per rank an int32 array (or None)."""
+    one); dest_slab: per rank an int32 array (or None); peer_sums0 / peer_sums1: per rank the addresses ufs_dvm_sums_dev
+    returns on that rank (both or neither)."""
     n = len(peer_f0)
     keep = [None if d is None else np.ascontiguousarray(d, np.int32) for d in dest_slab]
-    a0 = (C.c_void_p * n)(*[C.c_void_p(x) for x in peer_f0])
-    a1 = (C.c_void_p * n)(*[C.c_void_p(x) for x in peer_f1])
+    arr = lambda xs: None if xs is None else (C.c_void_p * n)(*[C.c_void_p(x) for x in xs])
     ad = (C.c_void_p * n)(*[C.c_void_p(None if d is None else d.ctypes.data) for d in keep])
-    _check(h, lib().ufs_dvm_halo_push_setup(h, a0, a1, ad))
+    _check(h, lib().ufs_dvm_halo_push_setup(h, arr(peer_f0), arr(peer_f1), ad, arr(peer_sums0), arr(peer_sums1)))
+
+
+def ufs_dvm_sums_dev(h):
+    s0, s1 = C.c_void_p(), C.c_void_p()
+    _check(h, lib().ufs_dvm_sums_dev(h, C.byref(s0), C.byref(s1)))
+    return s0.value, s1.value
 
 
 def ufs_dvm_push_entries(h) -> dict:
     n, nt = C.c_int64(), C.c_int64()
-    _check(h, lib().ufs_dvm_push_entries(h, C.byref(n), C.byref(nt), None, None, None, None))
+    _check(h, lib().ufs_dvm_push_entries(h, C.byref(n), C.byref(nt), None, None, None, None, None, None))
     slab, mask = np.empty(n.value, np.int32), np.empty(n.value, np.uint8)
-    d0, d1 = np.empty(n.value, np.uint64), np.empty(n.value, np.uint64)
-    _check(h, lib().ufs_dvm_push_entries(h, None, None, slab.ctypes.data, mask.ctypes.data, d0.ctypes.data, d1.ctypes.data))
-    return {"n_push_tiles": int(nt.value), "slab": slab, "mask": mask, "dst0": d0, "dst1": d1}
+    d0, d1, s0, s1 = (np.empty(n.value, np.uint64) for _ in range(4))
+    _check(h, lib().ufs_dvm_push_entries(h, None, None, slab.ctypes.data, mask.ctypes.data, d0.ctypes.data, d1.ctypes.data,
+                                         s0.ctypes.data, s1.ctypes.data))
+    return {"n_push_tiles": int(nt.value), "slab": slab, "mask": mask, "dst0": d0, "dst1": d1, "sums0": s0, "sums1": s1}
 
 
 def ufs_dvm_tiles(h) -> dict:

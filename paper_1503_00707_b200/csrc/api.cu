@@ -46,9 +46,12 @@ struct ufs_dvm_s {
     // partitioned mesh: per peer the chunk lists (slab * 8 + octant) to send / to receive, on the device
     std::vector<int32_t*> d_send_chunks, d_recv_chunks;
     std::vector<int64_t> n_send_chunks, n_recv_chunks;
+    std::vector<int32_t*> d_send_slabs, d_recv_slabs;   // ... and the slab lists themselves (the cells' sums travel too)
     bool check = false;            // UFS_DVM_CHECK: every step call verifies the carried sums of a few cells against f
     double* d_check = nullptr;     // scratch of the check
     uint64_t check_rng = 0x9E3779B97F4A7C15ull;
+    bool push_sums = false;        // fused exchange: the peers' step kernels also write the ghost cells' sums
+    bool ghost_sums_pushed = false; // the ghost rows of the sums hold the owners' sums of the current f (unpacked, or pushed)
     bool ghosts_fresh = false;     // the ghost slabs of f[cur] and their sums are those of the peers' current f
     bool sums_valid = false;       // d_sums[cur] describes f[cur]
     int parity = 0;
@@ -257,9 +260,11 @@ int ufs_dvm_create_part(const ufs_dvm_desc* desc, const int32_t* rank_of_leaf, i
     // chunk lists per peer
     h->d_send_chunks.assign(m.n_ranks, nullptr); h->d_recv_chunks.assign(m.n_ranks, nullptr);
     h->n_send_chunks.assign(m.n_ranks, 0); h->n_recv_chunks.assign(m.n_ranks, 0);
+    h->d_send_slabs.assign(m.n_ranks, nullptr); h->d_recv_slabs.assign(m.n_ranks, nullptr);
     for (int pr = 0; pr < m.n_ranks; pr++)
         for (int dir = 0; dir < 2; dir++) {
             const std::vector<int32_t>& slab = dir ? m.recv_slab[pr] : m.send_slab[pr];
+            if ((rc = upload(h, dir ? &h->d_recv_slabs[pr] : &h->d_send_slabs[pr], slab.data(), slab.size() * 4, "upload halo slab lists"))) return rc;
             const std::vector<uint8_t>& mask = dir ? m.recv_mask[pr] : m.send_mask[pr];
             std::vector<int32_t> chunks;
             for (size_t i = 0; i < slab.size(); i++)
@@ -423,6 +428,7 @@ int ufs_dvm_step(ufs_dvm_t h, double dt, int nsteps) {
         const int nl = h->plan.ring == 4 ? tiles_launches_per_step(plan, p) : 1;
         if (nl & 1) h->parity ^= 1;
         if (has_ghosts) h->ghosts_fresh = false;
+        h->ghost_sums_pushed = h->plan.push_on && h->push_sums;   // by the peers' step kernels of this round (protocol: ufs_dvm.h)
         if (h->mesh.n_kin > 0) h->launches += ((stream && p.collide) ? 1 : 0) + nl;
     }
     return UFS_DVM_OK;
@@ -478,6 +484,8 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         cudaFree(h->d_check); cudaFree(h->d_tile_push); cudaFree(h->d_ghost_tiles);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
         for (int32_t* q : h->d_recv_chunks) cudaFree(q);
+        for (int32_t* q : h->d_send_slabs) cudaFree(q);
+        for (int32_t* q : h->d_recv_slabs) cudaFree(q);
         for (auto& pr : h->prof_ev) for (cudaEvent_t e : pr) if (e) cudaEventDestroy(e);
     }
     delete h;
@@ -665,8 +673,10 @@ int ufs_dvm_halo_bytes(ufs_dvm_t h, int32_t peer, int64_t* send_bytes, int64_t* 
     int64_t ns = 0, nr = 0;
     for (uint8_t mk : m.send_mask[peer]) ns += __builtin_popcount(mk);
     for (uint8_t mk : m.recv_mask[peer]) nr += __builtin_popcount(mk);
-    if (send_bytes) *send_bytes = ns * chunk_bytes_of(h);
-    if (recv_bytes) *recv_bytes = nr * chunk_bytes_of(h);
+    // behind the chunks: the 36 carried sums of every listed cell (streaming kernels; the one-CTA-per-cell kernels carry none)
+    const int64_t tail = h->plan.ring >= 2 ? (int64_t)(SUMS_STRIDE * sizeof(double)) : 0;
+    if (send_bytes) *send_bytes = ns * chunk_bytes_of(h) + (int64_t)m.send_slab[peer].size() * tail;
+    if (recv_bytes) *recv_bytes = nr * chunk_bytes_of(h) + (int64_t)m.recv_slab[peer].size() * tail;
     return UFS_DVM_OK;
 }
 
@@ -682,6 +692,18 @@ static int halo_copy(ufs_dvm_t h, int32_t peer, void* buf, bool pack) {
     CU(launch_halo_copy(pack, pack ? h->d_send_chunks[peer] : h->d_recv_chunks[peer], n, h->f[h->cur], buf, chunk_bytes_of(h), h->stream),
        "halo copy kernel launch");
     h->launches++;
+    if (h->plan.ring >= 2) {
+        // the cells' carried sums behind the chunks (a sender that has not summed its f yet does so now)
+        if (pack && !h->sums_valid) {
+            const int rc = enqueue_sums(h, make_params(h, 1.0));
+            if (rc) return rc;
+        }
+        const int64_t n_slabs = (int64_t)(pack ? m.send_slab[peer].size() : m.recv_slab[peer].size());
+        CU(launch_halo_sums(pack, pack ? h->d_send_slabs[peer] : h->d_recv_slabs[peer], n_slabs, h->d_sums[h->cur],
+                            static_cast<char*>(buf) + n * chunk_bytes_of(h), h->stream), "halo sums kernel launch");
+        h->launches++;
+        if (!pack) h->ghost_sums_pushed = true;   // the ghost rows hold the owners' sums: nothing for ufs_dvm_halo_done to form
+    }
     return UFS_DVM_OK;
 }
 int ufs_dvm_halo_pack(ufs_dvm_t h, int32_t peer, void* buf_dev) { return halo_copy(h, peer, buf_dev, true); }
@@ -693,7 +715,7 @@ int ufs_dvm_halo_done(ufs_dvm_t h) {
     if (h->sticky) return h->sticky;
     const FlatMesh& m = h->mesh;
     const int64_t n_gh = m.n_slabs - m.n_kin;
-    if (n_gh > 0 && h->plan.ring >= 2) {
+    if (n_gh > 0 && h->plan.ring >= 2 && !h->ghost_sums_pushed) {
         // the velocity sums of the ghost cells, from the chunks that have just arrived (the step's Maxwellian needs
         // the upwind flux moments of every source; entries of chunks that never arrive are never read)
         StepParams p = make_params(h, 1.0);
@@ -715,7 +737,16 @@ int ufs_dvm_halo_done(ufs_dvm_t h) {
     return UFS_DVM_OK;
 }
 
-int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer_f1, const int32_t* const* dest_slab) {
+int ufs_dvm_sums_dev(ufs_dvm_t h, void** sums0, void** sums1) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (sums0) *sums0 = h->d_sums[0];
+    if (sums1) *sums1 = h->d_sums[1];
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer_f1, const int32_t* const* dest_slab,
+                            void* const* peer_sums0, void* const* peer_sums1) {
     if (!h) return UFS_DVM_EINVAL;
     if (h->sticky) return h->sticky;
     if (!h->mesh.partial) return fail(h, UFS_DVM_EINVAL, "not a partitioned mesh");
@@ -726,13 +757,17 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer
     std::string err;
     int rc;
     try {
-        rc = build_push(m, peer_f0, peer_f1, dest_slab, (int64_t)(m.vel.Nv * elem), err);
+        if ((peer_sums0 == nullptr) != (peer_sums1 == nullptr)) return fail(h, UFS_DVM_EINVAL, "peer_sums0 and peer_sums1: both or neither");
+        rc = build_push(m, peer_f0, peer_f1, dest_slab, (int64_t)(m.vel.Nv * elem), peer_sums0, peer_sums1,
+                        (int64_t)(SUMS_STRIDE * sizeof(double)), err);
     } catch (const std::bad_alloc&) {
         return fail(h, UFS_DVM_ENOMEM, "out of host memory");
     }
     if (rc) return fail(h, rc, err);
     h->plan.push_on = 1;
     h->plan.push_tiles = (int32_t)m.n_push_tiles;
+    h->push_sums = peer_sums0 != nullptr;
+    h->ghost_sums_pushed = false;
     if (!h->device) return UFS_DVM_OK;   // host-only handle: the records are built (ufs_dvm_push_entries), nothing to upload
     CU(cudaStreamSynchronize(h->stream), "stream synchronize");   // no step in flight reads the old headers
     cudaFree(h->d_tile_push);
@@ -746,7 +781,8 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void* const* peer_f0, void* const* peer
     return UFS_DVM_OK;
 }
 
-int ufs_dvm_push_entries(ufs_dvm_t h, int64_t* n_entries, int64_t* n_push_tiles, int32_t* slab, uint8_t* mask, uint64_t* dst0, uint64_t* dst1) {
+int ufs_dvm_push_entries(ufs_dvm_t h, int64_t* n_entries, int64_t* n_push_tiles, int32_t* slab, uint8_t* mask, uint64_t* dst0, uint64_t* dst1,
+                         uint64_t* sums0, uint64_t* sums1) {
     if (!h) return UFS_DVM_EINVAL;
     const FlatMesh& m = h->mesh;
     if (!h->plan.push_on) return fail(h, UFS_DVM_EINVAL, "ufs_dvm_halo_push_setup has not been called");
@@ -760,6 +796,8 @@ int ufs_dvm_push_entries(ufs_dvm_t h, int64_t* n_entries, int64_t* n_push_tiles,
                 if (mask) mask[e] = (uint8_t)(m.tile_push[e].info & 0xffu);
                 if (dst0) dst0[e] = m.tile_push[e].dst[0];
                 if (dst1) dst1[e] = m.tile_push[e].dst[1];
+                if (sums0) sums0[e] = m.tile_push[e].sums_dst[0];
+                if (sums1) sums1[e] = m.tile_push[e].sums_dst[1];
             }
     }
     return UFS_DVM_OK;

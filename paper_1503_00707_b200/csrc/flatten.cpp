@@ -704,7 +704,7 @@ void build_tiles(FlatMesh& m, int pmax) {
 }
 
 int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_f1, const int32_t* const* dest_slab, int64_t slab_bytes,
-               std::string& err) {
+               const void* const* peer_sums0, const void* const* peer_sums1, int64_t sums_row_bytes, std::string& err) {
     if (!m.partial) { err = "fused ghost exchange: not a partitioned mesh"; return UFS_DVM_EINVAL; }
     if (m.tiles.empty() && m.n_kin > 0) { err = "fused ghost exchange: needs the tile kernel (k_tiles)"; return UFS_DVM_EINVAL; }
     // per inner slab: the peers that need it
@@ -722,6 +722,14 @@ int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_
             PushEntry e{};
             e.dst[0] = (uint64_t)(uintptr_t)peer_f0[pr] + (uint64_t)d * (uint64_t)slab_bytes;
             e.dst[1] = (uint64_t)(uintptr_t)peer_f1[pr] + (uint64_t)d * (uint64_t)slab_bytes;
+            if (peer_sums0 && peer_sums1) {
+                if (!peer_sums0[pr] || !peer_sums1[pr]) {
+                    err = "fused ghost exchange: the sums arrays of rank " + std::to_string(pr) + " are NULL";
+                    return UFS_DVM_EINVAL;
+                }
+                e.sums_dst[0] = (uint64_t)(uintptr_t)peer_sums0[pr] + (uint64_t)d * (uint64_t)sums_row_bytes;
+                e.sums_dst[1] = (uint64_t)(uintptr_t)peer_sums1[pr] + (uint64_t)d * (uint64_t)sums_row_bytes;
+            }
             e.info = m.send_mask[pr][i];
             if ((e.dst[0] | e.dst[1]) & 15) { err = "fused ghost exchange: peer buffers must be 16-byte aligned"; return UFS_DVM_EINVAL; }
             of_slab[s].push_back(e);

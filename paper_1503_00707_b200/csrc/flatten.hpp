@@ -94,12 +94,13 @@ static_assert(sizeof(TileHdr) == 32, "TileHdr must be 32 bytes");
 // into that peer's ghost slab of the NEXT f.  One entry per (cell, peer); a tile's entries are consecutive, ordered by
 // cell: TileHdr::pad[0] = index of the tile's first entry, pad[1] = eight 4-bit counts (entries of cell c in bits 4c..4c+3).
 constexpr int PUSH_PER_CELL_MAX = 4;           // peers that may need one cell (more: the pack / unpack exchange serves)
-struct PushEntry {                             // 32 bytes
+struct PushEntry {                             // 48 bytes
     uint64_t dst[2];                           // address of the peer's ghost slab in its f buffer 0 / 1 (peer memory)
+    uint64_t sums_dst[2];                      // address of that ghost cell's 36 velocity sums in the peer's sums array 0 / 1, or 0
     uint32_t info;                             // bits 0..7: octant mask of the chunks the peer needs
     uint32_t pad[3];
 };
-static_assert(sizeof(PushEntry) == 32, "PushEntry must be 32 bytes");
+static_assert(sizeof(PushEntry) == 48, "PushEntry must be 48 bytes");
 
 struct FlatMesh {
     int64_t n_leaves = 0, n_kin = 0;
@@ -187,7 +188,9 @@ void build_tiles(FlatMesh& m, int pmax);
 // (m.n_push_tiles of them) and fills m.tile_push and the pad words of m.tiles from the send lists.  Per peer
 // rank p: peer_f[b][p] = address (as this device reaches it) of rank p's f buffer b, dest_slab[p][i] = the ghost slab of
 // rank p that takes this rank's i-th send slab (rank p's recv_slab list for this rank), slab_bytes = Nv * element size.
+// peer_sums[b] (may be NULL): per peer the address of its velocity-sums array b ([slabs][sums_stride] doubles): the owner's
+// sums of a pushed cell then go to the peer's ghost row as well.
 int build_push(FlatMesh& m, const void* const* peer_f0, const void* const* peer_f1, const int32_t* const* dest_slab, int64_t slab_bytes,
-               std::string& err);
+               const void* const* peer_sums0, const void* const* peer_sums1, int64_t sums_row_bytes, std::string& err);
 
 }  // namespace ufs

@@ -109,6 +109,8 @@ cudaError_t launch_remap(int storage, const void* f_old, void* f_new, const int6
 
 // halo.cu: ghost-cell exchange of a partitioned mesh: chunk list -> contiguous buffer (pack) or back (unpack)
 cudaError_t launch_halo_copy(bool pack, const int32_t* chunks, int64_t n_chunks, void* f, void* buf, int64_t chunk_bytes, cudaStream_t stream);
+// ... and the listed cells' carried sums <-> the tail of the buffer ([n_slabs][SUMS_STRIDE] doubles)
+cudaError_t launch_halo_sums(bool pack, const int32_t* slabs, int64_t n_slabs, double* sums, void* tail, cudaStream_t stream);
 
 // Enqueue one fused step (transport + moments + discrete Maxwellian + relaxation) on `stream`.
 cudaError_t launch_step(int storage, const StepLaunch& plan, const StepParams& p, cudaStream_t stream);

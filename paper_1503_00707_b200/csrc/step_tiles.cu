@@ -676,7 +676,21 @@ __global__ void __launch_bounds__((N_PROD + N_CONS) * 32, 1) k_tiles(const StepP
                 const int cc = 2 * triple + u / SUMS_STRIDE, j = u % SUMS_STRIDE;
                 if (cc < nc) {
                     const double* rp = reinterpret_cast<const double*>(smem_raw + o_red) + (size_t)(n & 1) * RED_DOUBLES + (size_t)cc * 3 * SUMS_STRIDE + j;
-                    p.sums_out[(int64_t)(s0 + cc) * SUMS_STRIDE + j] = rp[0] + rp[SUMS_STRIDE] + rp[2 * SUMS_STRIDE];
+                    const double sum = rp[0] + rp[SUMS_STRIDE] + rp[2 * SUMS_STRIDE];
+                    p.sums_out[(int64_t)(s0 + cc) * SUMS_STRIDE + j] = sum;
+                    if constexpr (PUSH) {
+                        // the peers that hold this cell as a ghost cell get its sums too (their k_prep reads them as an upwind source's)
+                        const uint32_t cnts = *reinterpret_cast<const uint32_t*>(smem_raw + hdr + 28);
+                        const int pc = (int)((cnts >> (4 * cc)) & 15u);
+                        if (pc) {
+                            int first = *reinterpret_cast<const int*>(smem_raw + hdr + 24);
+                            for (int i = 0; i < cc; i++) first += (int)((cnts >> (4 * i)) & 15u);
+                            for (int e = 0; e < pc; e++) {
+                                const unsigned long long d = __ldg(reinterpret_cast<const unsigned long long*>(p.tile_push[first + e].sums_dst) + p.push_parity);
+                                if (d) reinterpret_cast<double*>(d)[j] = sum;
+                            }
+                        }
+                    }
                 }
             }
         }

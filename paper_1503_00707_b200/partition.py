@@ -78,12 +78,13 @@ class RankStepper(B.DvmStepper):
     def halo_done(self):
         B.ufs_dvm_halo_done(self.h)
 
-    def setup_push(self, peer_f, dest_slab):
+    def setup_push(self, peer_f, dest_slab, peer_sums=None):
         """Switch this rank to the fused ghost exchange (ufs_dvm_halo_push_setup): peer_f[p] = (address of rank p's f
         buffer 0, of its buffer 1) as this device reaches them, dest_slab[p] = rank p's recv_slab list for this rank;
-        None for ranks that need nothing from this one."""
-        B.ufs_dvm_halo_push_setup(self.h, [None if x is None else x[0] for x in peer_f], [None if x is None else x[1] for x in peer_f],
-                                  dest_slab)
+        None for ranks that need nothing from this one.  peer_sums[p] = rank p's ufs_dvm_sums_dev pair: the ghost cells'
+        sums are pushed as well."""
+        pick = lambda xs, b: None if xs is None else [None if x is None else x[b] for x in xs]
+        B.ufs_dvm_halo_push_setup(self.h, pick(peer_f, 0), pick(peer_f, 1), dest_slab, pick(peer_sums, 0), pick(peer_sums, 1))
         self.push = True
 
     def halo_bytes(self):
@@ -143,17 +144,19 @@ def exchange_distributed(rank: RankStepper, group=None):
         rank.halo_done()
 
 
-def setup_push_local(ranks: List[RankStepper]):
+def setup_push_local(ranks: List[RankStepper], push_sums: bool = True):
     """Fused ghost exchange between ranks emulated on ONE device: every rank's step kernel stores its boundary cells
-    straight into the other ranks' ghost slabs (the same address space: the peers' own pointers)."""
+    straight into the other ranks' ghost slabs (the same address space: the peers' own pointers), and with push_sums their
+    velocity sums into the other ranks' sums arrays."""
     n = len(ranks)
     for r in ranks:
-        peer_f, dest = [None] * n, [None] * n
+        peer_f, dest, sums = [None] * n, [None] * n, [None] * n
         for p in r.peers:
             if B.ufs_dvm_halo_bytes(r.h, p)[0]:
                 peer_f[p] = (ranks[p].f[0].data_ptr(), ranks[p].f[1].data_ptr())
                 dest[p] = B.ufs_dvm_halo(ranks[p].h, r.my_rank)["recv_slab"]
-        r.setup_push(peer_f, dest)
+                sums[p] = B.ufs_dvm_sums_dev(ranks[p].h)
+        r.setup_push(peer_f, dest, sums if push_sums else None)
 
 
 def step_pushed_local(ranks: List[RankStepper], dt: float):
@@ -169,7 +172,8 @@ def setup_push_distributed(rank: RankStepper, group=None):
     """Fused ghost exchange between real ranks of one node.  The two f tensors of `rank` must have been allocated by
     torch.distributed._symmetric_memory.empty (rank.f_symm = the two rendezvous handles): every rank's buffers are then
     mapped into every other rank's address space over NVLink, and the peers' recv_slab lists travel once, on the host,
-    by all_gather_object."""
+    by all_gather_object.  (The ghost cells' sums are not pushed here: the sums arrays are the library's own allocations,
+    and mapping them into another process takes cudaIpc handles; ufs_dvm_halo_done sums the ghost slabs instead.)"""
     import torch.distributed as dist
     n = rank.n_ranks
     mine = {p: B.ufs_dvm_halo(rank.h, p)["recv_slab"] for p in rank.peers}

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 TOL = {inputs.STORE_F64: 1e-12, inputs.STORE_F32: 2e-5}
 
 
-def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False):
+def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False, push_sums=True):
     desc, keep = B.make_desc(case)
     rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, w_fluid)
     f0 = inputs.initial_f(case)
@@ -32,13 +32,14 @@ def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False):
         if push:
             # fused exchange: one ordinary exchange for the first step's ghosts, from then on the step kernels write the
             # boundary cells into the peers' ghost slabs themselves -- no pack, copy or unpack launch after this point
-            setup_push_local(ranks)
+            setup_push_local(ranks, push_sums=push_sums)
             exchange_local(ranks)
             before = [B.ufs_dvm_launch_count(r.h) for r in ranks]
             for _ in range(nsteps):
                 step_pushed_local(ranks, case.dt)
             for r, b in zip(ranks, before):
-                per_step = 3 + (1 if r.n_ghost else 0)         # k_prep, k_tiles on the boundary tiles, on the rest, ghost sums
+                # k_prep, k_tiles on the boundary tiles, k_tiles on the rest; the ghost sums only if the peers do not push them
+                per_step = 3 + (1 if r.n_ghost and not push_sums else 0)
                 first = 1 if r.n_inner else 0                  # the sums pass of the initial f
                 assert B.ufs_dvm_launch_count(r.h) - b <= nsteps * per_step + first
         else:
@@ -127,13 +128,15 @@ def test_partitioned_config3_at_stated_size_four_ranks(push):
     assert_moments_close(mom, o.moments(f_ref), 1e-12)
 
 
-@pytest.mark.parametrize("cfg,n_ranks", [(3, 2), (3, 3), (4, 2), (4, 4), (5, 3)])
-def test_fused_exchange_matches_the_one_domain_oracle(cfg, n_ranks):
+@pytest.mark.parametrize("cfg,n_ranks,push_sums", [(3, 2, True), (3, 3, False), (4, 2, True), (4, 4, False), (5, 3, True),
+                                                   (5, 3, False)])
+def test_fused_exchange_matches_the_one_domain_oracle(cfg, n_ranks, push_sums):
     """ufs_dvm_halo_push_setup: the step kernel stores the boundary cells into the peers' ghost slabs (peer memory; here the
-    ranks share one device) -- 2:1 faces, walls, a SOLID body, the kinetic/fluid mask (k_tiles' FLUID instantiation), fp32."""
+    ranks share one device) -- 2:1 faces, walls, a SOLID body, the kinetic/fluid mask (k_tiles' FLUID instantiation), fp32;
+    with the cells' sums pushed as well, or formed from the ghost slabs by ufs_dvm_halo_done."""
     case = inputs.small(cfg)
     nsteps = 4
-    f0, f, mom, sent = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=True)
+    f0, f, mom, sent = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=True, push_sums=push_sums)
     o = Oracle(case)
     f_ref = o.step(f0, case.dt, nsteps)
     tol = TOL[case.storage]
@@ -143,12 +146,34 @@ def test_fused_exchange_matches_the_one_domain_oracle(cfg, n_ranks):
 
 
 def test_fused_exchange_is_bit_equal_to_the_packed_exchange():
-    """The same rows reach the same ghost slabs either way: the two exchanges give bit-identical fields."""
+    """The same rows reach the same ghost slabs and the same owner's sums reach the same ghost rows either way: the two
+    exchanges give bit-identical fields."""
     case = inputs.small(3)
     _, f_a, mom_a, _ = _run_partitioned(case, 3, 3)
     _, f_b, mom_b, _ = _run_partitioned(case, 3, 3, push=True)
     assert np.array_equal(f_a, f_b)
     assert np.array_equal(mom_a, mom_b)
+
+
+@pytest.mark.parametrize("push", [False, True])
+@pytest.mark.parametrize("cfg,n_ranks", [(3, 3), (4, 2), (5, 3)])
+def test_partitioned_run_is_bit_identical_to_the_one_domain_run(cfg, n_ranks, push):
+    """The ghost rows of the sums hold the owners' own carried sums (behind the chunks of the packed exchange, or pushed by
+    the peers' step kernels), so a cell sees exactly what it sees in the unpartitioned run -- the same f in its upwind
+    sources, the same sums behind its Maxwellian -- and the stitched field is the one-domain device run bit for bit
+    (walls, SOLID body, 2:1 faces; fp32 storage; the kinetic/fluid mask)."""
+    case = inputs.small(cfg)
+    nsteps = 4
+    f0, f, mom, _ = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=push)
+    st = B.DvmStepper(case)
+    try:
+        st.load_canonical(f0)
+        st.step(case.dt, nsteps)
+        st.sync()
+        assert np.array_equal(st.read_canonical(), f)
+        assert np.array_equal(st.moments(), mom)
+    finally:
+        st.close()
 
 
 def test_fused_exchange_push_entries_cover_the_send_lists():

@@ -124,7 +124,9 @@ def test_halo_lists_equal_the_brute_force_derivation(name, n_ranks):
                 sb, _ = B.ufs_dvm_halo_bytes(hs[p], r)
                 _, rb = B.ufs_dvm_halo_bytes(hs[r], p)
                 chunk = (case.Nv // 8) * 8
-                assert sb == rb == sum(bin(m).count("1") for _, m in sent) * chunk
+                # chunks, then (streaming kernels) the 36 carried sums of every listed cell
+                tail = 36 * 8 if B.ufs_dvm_kernel_name(hs[p]) in ("k_tiles", "k_rows", "k_stream") else 0
+                assert sb == rb == sum(bin(m).count("1") for _, m in sent) * chunk + len(sent) * tail
             assert set(ghosts.tolist()) == set(want_all)              # no ghost nobody reads, none missing
             if want_all:
                 assert max(bin(m).count("1") for m in want_all.values()) <= 8
@@ -164,8 +166,18 @@ def test_push_entries_pair_every_send_slab_with_the_peers_ghost_slab(name, n_ran
             with pytest.raises(B.UfsDvmError):
                 B.ufs_dvm_push_entries(hs[r])                       # not set up yet
             dest = [None if p == r else B.ufs_dvm_halo(hs[p], r)["recv_slab"] for p in range(n_ranks)]
+            sbase = lambda p, b: base(p, b) + (1 << 30)
             B.ufs_dvm_halo_push_setup(hs[r], [None if p == r else base(p, 0) for p in range(n_ranks)],
                                       [None if p == r else base(p, 1) for p in range(n_ranks)], dest)
+            assert not B.ufs_dvm_push_entries(hs[r])["sums0"].any()          # no sums arrays given: no sums pushed
+            with pytest.raises(B.UfsDvmError):                              # both or neither
+                B.ufs_dvm_halo_push_setup(hs[r], [None if p == r else base(p, 0) for p in range(n_ranks)],
+                                          [None if p == r else base(p, 1) for p in range(n_ranks)], dest,
+                                          [None if p == r else sbase(p, 0) for p in range(n_ranks)], None)
+            B.ufs_dvm_halo_push_setup(hs[r], [None if p == r else base(p, 0) for p in range(n_ranks)],
+                                      [None if p == r else base(p, 1) for p in range(n_ranks)], dest,
+                                      [None if p == r else sbase(p, 0) for p in range(n_ranks)],
+                                      [None if p == r else sbase(p, 1) for p in range(n_ranks)])
             ent = B.ufs_dvm_push_entries(hs[r])
             want = set()
             for p in range(n_ranks):
@@ -173,8 +185,10 @@ def test_push_entries_pair_every_send_slab_with_the_peers_ghost_slab(name, n_ran
                     continue
                 hl = B.ufs_dvm_halo(hs[r], p)
                 for s, m, d in zip(hl["send_slab"], hl["send_mask"], dest[p]):
-                    want.add((int(s), int(m), base(p, 0) + int(d) * slab_bytes, base(p, 1) + int(d) * slab_bytes))
-            got = list(zip(ent["slab"].tolist(), ent["mask"].tolist(), ent["dst0"].tolist(), ent["dst1"].tolist()))
+                    want.add((int(s), int(m), base(p, 0) + int(d) * slab_bytes, base(p, 1) + int(d) * slab_bytes,
+                              sbase(p, 0) + int(d) * 36 * 8, sbase(p, 1) + int(d) * 36 * 8))    # a sums row: 36 doubles
+            got = list(zip(ent["slab"].tolist(), ent["mask"].tolist(), ent["dst0"].tolist(), ent["dst1"].tolist(),
+                           ent["sums0"].tolist(), ent["sums1"].tolist()))
             assert len(got) == len(set(got)) and set(got) == want
             t = B.ufs_dvm_tiles(hs[r])
             sent = np.zeros(B.ufs_dvm_part_layout(hs[r])["n_inner"], bool)
@@ -189,6 +203,7 @@ def test_push_entries_pair_every_send_slab_with_the_peers_ghost_slab(name, n_ran
                                       [None if p == r else base(p, 1) for p in range(n_ranks)], dest)
             ent2 = B.ufs_dvm_push_entries(hs[r])
             assert all(np.array_equal(ent[k], ent2[k]) for k in ("slab", "mask", "dst0", "dst1"))
+            assert not ent2["sums0"].any()
     finally:
         for h in hs:
             B.ufs_dvm_destroy(h)
