@@ -148,6 +148,36 @@ def aggregate_over_ranks(ms_local: float, units_local: float, device=None):
     return float(t.item()), float(u.item())
 
 
+def sustained_copy_gbs(torch, dev, seconds=1.0):
+    """Read + write bytes per second of b.copy_(a) over 2 x 2 GiB (the recipe behind MEASURED_PEAKS.json's hbm_gbs), best of
+    the first ten copies and the mean over about `seconds` of back-to-back copies, on torch's current stream."""
+    n = 1 << 30
+    a = torch.empty(n, dtype=torch.int16, device=dev).zero_()
+    b = torch.empty_like(a)
+    for _ in range(3):
+        b.copy_(a)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(11)]
+    ev[0].record()
+    for i in range(10):
+        b.copy_(a)
+        ev[i + 1].record()
+    torch.cuda.synchronize(dev)
+    burst_ms = min(ev[i].elapsed_time(ev[i + 1]) for i in range(10))
+    reps = max(10, int(seconds * 1e3 / burst_ms))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        b.copy_(a)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    bytes_per_copy = 2.0 * n * 2
+    out = {"burst_GBs": bytes_per_copy / (burst_ms * 1e-3) / 1e9,
+           "sustained_GBs": bytes_per_copy * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9, "sustained_copies": reps,
+           "what": "torch b.copy_(a), 2 GiB read + 2 GiB written per copy, after the timed steps"}
+    del a, b
+    return out
+
+
 def run_partitioned(args):
     """The partitioned step (include/ufs_dvm.h "Partitioned mesh"): the workload cut along the
     N-order curve into equal-weight ranks, ghost chunks exchanged before every step.  Under torchrun every process is
@@ -351,6 +381,7 @@ def main():
     ap.add_argument("--fused-exchange", action="store_true",
                     help="partitioned step: the step kernel writes the peers' ghost slabs itself (ufs_dvm_halo_push_setup)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-copy-context", action="store_true", help="skip the plain-copy bandwidth measured beside the roofline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -437,6 +468,15 @@ def main():
     ms, updates_all = aggregate_over_ranks(ms, float(n_kin * Nv * args.steps), dev)
     value = updates_all / (ms * 1e-3)
 
+    # ---- context for the roofline: what a plain device copy sustains on this box right now (MEASURED_PEAKS.json holds the
+    # burst figure, best of ten copies on a cool device; a long step runs under the power cap)
+    copy_ctx = None
+    if rank == 0 and not args.no_copy_context:
+        try:
+            copy_ctx = sustained_copy_gbs(torch, dev)
+        except Exception as ex:  # not enough free device memory beside f, etc.
+            copy_ctx = {"unavailable": f"{type(ex).__name__}: {ex}"[:160]}
+
     # ---- roofline of the dominant kernel (the streaming pass over f): its own launches, timed by events ----
     peak, peak_src = peaks()
     alg_bytes_per_launch = 2.0 * n_kin * Nv * elem          # 1 read + 1 write of f per phase-space cell
@@ -452,6 +492,10 @@ def main():
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch,
                 "whole_step_GBs": alg_bytes_per_launch / (ms * 1e-3 / args.steps) / 1e9,
                 "frac_of_8TBs_nominal": achieved / 8000.0}
+    if copy_ctx is not None:
+        roofline["copy_on_this_box"] = copy_ctx
+        if copy_ctx.get("sustained_GBs"):
+            roofline["frac_of_sustained_copy"] = achieved / copy_ctx["sustained_GBs"]
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
