@@ -270,6 +270,13 @@ int ufs_dvm_halo_push_setup(ufs_dvm_t h, void *const *peer_f0, void *const *peer
  * themselves with peer access enabled; another process: their cudaIpcOpenMemHandle mappings). */
 int ufs_dvm_sums_dev(ufs_dvm_t h, void **sums0, void **sums1);
 
+/* Make the handle keep its carried sums in two CALLER-owned DEVICE arrays, each (n_inner + n_ghost) * 36 doubles, 16-byte
+ * aligned, instead of its own allocations (whose contents are copied over; the call synchronises the stream).  For ranks in
+ * different processes: arrays from a symmetric allocation are mapped into every peer by the allocator's rendezvous, which
+ * the library's own cudaMalloc'ed arrays are not; the peers' mappings are then the peer_sums0 / peer_sums1 of
+ * ufs_dvm_halo_push_setup.  The arrays must outlive the handle; ufs_dvm_destroy does not free them. */
+int ufs_dvm_sums_use(ufs_dvm_t h, void *sums0, void *sums1);
+
 /* The push entries that ufs_dvm_halo_push_setup built (it also accepts a host-only handle: the records are built, nothing
  * is uploaded; the addresses are then just numbers), in the order the kernel reads them (HOST outputs, any may be NULL):
  * *n_entries, *n_push_tiles (the tiles with entries: the first ones of ufs_dvm_tiles); per entry: slab = the inner slab whose

@@ -23,7 +23,7 @@ EXPORTS = ["ufs_dvm_create", "ufs_dvm_create_host", "ufs_dvm_step", "ufs_dvm_mom
            "ufs_dvm_last_error", "ufs_dvm_f_changed", "ufs_dvm_profile", "ufs_dvm_kernel_ms", "ufs_dvm_tiles", "ufs_dvm_remesh", "ufs_dvm_remap_plan",
            "ufs_dvm_partition", "ufs_dvm_create_part", "ufs_dvm_create_part_host", "ufs_dvm_part_layout", "ufs_dvm_halo",
            "ufs_dvm_halo_bytes", "ufs_dvm_halo_pack", "ufs_dvm_halo_unpack", "ufs_dvm_halo_done", "ufs_dvm_moments_static",
-           "ufs_dvm_halo_push_setup", "ufs_dvm_push_entries", "ufs_dvm_sums_dev"]
+           "ufs_dvm_halo_push_setup", "ufs_dvm_push_entries", "ufs_dvm_sums_dev", "ufs_dvm_sums_use"]
 
 STATIC_MAX_CELLS = 8192   # UFS_DVM_STATIC_MAX_CELLS of include/ufs_dvm.h
 
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
         L.ufs_dvm_halo_done.argtypes = [vp]
         L.ufs_dvm_halo_push_setup.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ufs_dvm_sums_dev.argtypes = [vp, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]
+        L.ufs_dvm_sums_use.argtypes = [vp, vp, vp]
         L.ufs_dvm_push_entries.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp, vp, vp, vp, vp, vp]
         L.ufs_dvm_launch_count.argtypes = [vp]; L.ufs_dvm_launch_count.restype = C.c_int64
         L.ufs_dvm_kernel_info.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
@@ -310,6 +311,10 @@ def ufs_dvm_halo_push_setup(h, peer_f0, peer_f1, dest_slab, peer_sums0=None, pee
     arr = lambda xs: None if xs is None else (C.c_void_p * n)(*[C.c_void_p(x) for x in xs])
     ad = (C.c_void_p * n)(*[C.c_void_p(None if d is None else d.ctypes.data) for d in keep])
     _check(h, lib().ufs_dvm_halo_push_setup(h, arr(peer_f0), arr(peer_f1), ad, arr(peer_sums0), arr(peer_sums1)))
+
+
+def ufs_dvm_sums_use(h, sums0_ptr: int, sums1_ptr: int):
+    _check(h, lib().ufs_dvm_sums_use(h, C.c_void_p(sums0_ptr), C.c_void_p(sums1_ptr)))
 
 
 def ufs_dvm_sums_dev(h):

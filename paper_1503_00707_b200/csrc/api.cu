@@ -33,6 +33,7 @@ struct ufs_dvm_s {
     int32_t* d_counter = nullptr;  // [2] cell counters of the ring kernel, one per launch parity
     // streaming step: velocity sums of f[0] / f[1], of the ghost states, and the per-step factor tables
     double* d_sums[2] = {nullptr, nullptr};
+    bool sums_are_callers = false;   // ufs_dvm_sums_use: the two arrays belong to the caller (not freed at destroy)
     double* d_ghost_sums = nullptr;
     void* d_tabs = nullptr;
     // tile kernel: the flattener's tile records
@@ -479,7 +480,8 @@ int ufs_dvm_destroy(ufs_dvm_t h) {
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) rc = UFS_DVM_ECUDA;
         cudaFree(h->d_cells); cudaFree(h->d_tables); cudaFree(h->d_fluid); cudaFree(h->d_vel);
         cudaFree(h->d_slot_k); cudaFree(h->d_mirror); cudaFree(h->d_flags); cudaFree(h->d_counter);
-        cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
+        if (!h->sums_are_callers) { cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); }
+        cudaFree(h->d_ghost_sums); cudaFree(h->d_tabs);
         cudaFree(h->d_tile_hdr); cudaFree(h->d_tile_pieces); cudaFree(h->d_tile_cellidx); cudaFree(h->d_fluid_pieces);
         cudaFree(h->d_check); cudaFree(h->d_tile_push); cudaFree(h->d_ghost_tiles);
         for (int32_t* q : h->d_send_chunks) cudaFree(q);
@@ -742,6 +744,25 @@ int ufs_dvm_sums_dev(ufs_dvm_t h, void** sums0, void** sums1) {
     if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
     if (sums0) *sums0 = h->d_sums[0];
     if (sums1) *sums1 = h->d_sums[1];
+    return UFS_DVM_OK;
+}
+
+int ufs_dvm_sums_use(ufs_dvm_t h, void* sums0, void* sums1) {
+    if (!h) return UFS_DVM_EINVAL;
+    if (!h->device) return fail(h, UFS_DVM_EINVAL, "host-only handle");
+    if (h->sticky) return h->sticky;
+    if (h->plan.ring < 2 || !h->d_sums[0]) return fail(h, UFS_DVM_EINVAL, "this handle carries no velocity sums");
+    if (!sums0 || !sums1 || sums0 == sums1 || ((uintptr_t)sums0 & 15) || ((uintptr_t)sums1 & 15))
+        return fail(h, UFS_DVM_EINVAL, "sums0 and sums1 must be two distinct 16-byte aligned device arrays");
+    // what the library's arrays hold (sums of the current f, ghost rows) moves over; then they are released
+    const size_t bytes = (size_t)h->mesh.n_slabs * SUMS_STRIDE * sizeof(double);
+    void* mine[2] = {sums0, sums1};
+    for (int b = 0; b < 2; b++) CU(cudaMemcpyAsync(mine[b], h->d_sums[b], bytes, cudaMemcpyDeviceToDevice, h->stream), "copy the sums");
+    CU(cudaStreamSynchronize(h->stream), "copy the sums");
+    if (!h->sums_are_callers) { cudaFree(h->d_sums[0]); cudaFree(h->d_sums[1]); }
+    h->d_sums[0] = static_cast<double*>(sums0);
+    h->d_sums[1] = static_cast<double*>(sums1);
+    h->sums_are_callers = true;
     return UFS_DVM_OK;
 }
 

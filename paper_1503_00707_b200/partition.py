@@ -36,14 +36,19 @@ class RankStepper(B.DvmStepper):
         self.n_inner, self.n_ghost = lay["n_inner"], lay["n_ghost"]
         n_slabs = self.n_inner + self.n_ghost
         with torch.cuda.device(self.device):
+            self.sums = None
             if symmetric:
                 self.f, self.f_symm = _symmetric_f(torch, n_slabs, self.Nv, self.dtype, self.device, group)
+                # the carried sums too (36 doubles per slab), so that the peers' step kernels can write the ghost rows
+                self.sums, self.sums_symm = _symmetric_f(torch, n_slabs, 36, torch.float64, self.device, group)
             else:
                 self.f = [torch.empty((n_slabs, self.Nv), dtype=self.dtype, device=self.device) for _ in range(2)]
             self.mom = torch.empty((5, max(self.n_inner, 1)), dtype=torch.float64, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self.h = B.ufs_dvm_create_part(desc, rank_of_leaf, my_rank, n_ranks, [t.data_ptr() for t in self.f],
                                            self.stream.cuda_stream)
+            if self.sums is not None:
+                B.ufs_dvm_sums_use(self.h, self.sums[0].data_ptr(), self.sums[1].data_ptr())
             self.peers = []
             self.send_buf, self.recv_buf = {}, {}
             elem = 4 if self.storage == STORE_F32 else 8
@@ -172,19 +177,20 @@ def setup_push_distributed(rank: RankStepper, group=None):
     """Fused ghost exchange between real ranks of one node.  The two f tensors of `rank` must have been allocated by
     torch.distributed._symmetric_memory.empty (rank.f_symm = the two rendezvous handles): every rank's buffers are then
     mapped into every other rank's address space over NVLink, and the peers' recv_slab lists travel once, on the host,
-    by all_gather_object.  (The ghost cells' sums are not pushed here: the sums arrays are the library's own allocations,
-    and mapping them into another process takes cudaIpc handles; ufs_dvm_halo_done sums the ghost slabs instead.)"""
+    by all_gather_object.  The carried sums live in symmetric memory as well (ufs_dvm_sums_use), so the ghost cells' sums
+    are pushed too."""
     import torch.distributed as dist
     n = rank.n_ranks
     mine = {p: B.ufs_dvm_halo(rank.h, p)["recv_slab"] for p in rank.peers}
     everyone = [None] * n
     dist.all_gather_object(everyone, mine, group=group)
-    peer_f, dest = [None] * n, [None] * n
+    peer_f, dest, sums = [None] * n, [None] * n, [None] * n
     for p in rank.peers:
         if B.ufs_dvm_halo_bytes(rank.h, p)[0]:
             peer_f[p] = tuple(int(rank.f_symm[b].buffer_ptrs[p]) for b in range(2))
+            sums[p] = tuple(int(rank.sums_symm[b].buffer_ptrs[p]) for b in range(2))
             dest[p] = everyone[p][rank.my_rank]
-    rank.setup_push(peer_f, dest)
+    rank.setup_push(peer_f, dest, sums)
     rank.push_token = rank.torch.zeros(1, dtype=rank.torch.int32, device=rank.device)
 
 

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 TOL = {inputs.STORE_F64: 1e-12, inputs.STORE_F32: 2e-5}
 
 
-def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False, push_sums=True):
+def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False, push_sums=True, own_sums=False):
     desc, keep = B.make_desc(case)
     rol = B.ufs_dvm_partition(desc, n_ranks, 1.0, w_fluid)
     f0 = inputs.initial_f(case)
@@ -25,9 +25,17 @@ def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False, push_sums=T
     kin = case.kinetic_leaves()
     glob_row = np.full(case.n_leaves, -1, np.int64); glob_row[kin] = np.arange(kin.size)
     ranks = [RankStepper(case, rol, r, n_ranks) for r in range(n_ranks)]
+    keep_sums = []
     try:
         for r in ranks:
             assert B.ufs_dvm_kernel_name(r.h) == "k_tiles"
+            if own_sums:
+                # the carried sums in caller-owned arrays (ufs_dvm_sums_use; what a symmetric allocation would be)
+                import torch
+                mine = [torch.full((r.n_inner + r.n_ghost, 36), float("nan"), dtype=torch.float64, device=r.device) for _ in range(2)]
+                B.ufs_dvm_sums_use(r.h, mine[0].data_ptr(), mine[1].data_ptr())
+                assert B.ufs_dvm_sums_dev(r.h) == (mine[0].data_ptr(), mine[1].data_ptr())
+                keep_sums.append(mine)
             r.load_canonical(f0[glob_row[r.inner_leaves]])
         if push:
             # fused exchange: one ordinary exchange for the first step's ghosts, from then on the step kernels write the
@@ -54,6 +62,10 @@ def _run_partitioned(case, n_ranks, nsteps, w_fluid=0.0, push=False, push_sums=T
             f[glob_row[r.inner_leaves]] = r.read_canonical()
             mom[:, glob_row[r.inner_leaves]] = r.moments()
         sent = sum(r.halo_bytes()[0] for r in ranks)
+        for r, mine in zip(ranks, keep_sums):
+            cur = B.ufs_dvm_current(r.h)
+            rows = mine[cur][:r.n_inner, :35].cpu().numpy()
+            assert np.all(np.isfinite(rows)) and np.all(rows[:, 0] > 0)     # the step kernel wrote the caller's arrays
         return f0, f, mom, sent
     finally:
         for r in ranks:
@@ -155,16 +167,16 @@ def test_fused_exchange_is_bit_equal_to_the_packed_exchange():
     assert np.array_equal(mom_a, mom_b)
 
 
-@pytest.mark.parametrize("push", [False, True])
+@pytest.mark.parametrize("push,own_sums", [(False, False), (True, False), (True, True)])
 @pytest.mark.parametrize("cfg,n_ranks", [(3, 3), (4, 2), (5, 3)])
-def test_partitioned_run_is_bit_identical_to_the_one_domain_run(cfg, n_ranks, push):
+def test_partitioned_run_is_bit_identical_to_the_one_domain_run(cfg, n_ranks, push, own_sums):
     """The ghost rows of the sums hold the owners' own carried sums (behind the chunks of the packed exchange, or pushed by
     the peers' step kernels), so a cell sees exactly what it sees in the unpartitioned run -- the same f in its upwind
     sources, the same sums behind its Maxwellian -- and the stitched field is the one-domain device run bit for bit
     (walls, SOLID body, 2:1 faces; fp32 storage; the kinetic/fluid mask)."""
     case = inputs.small(cfg)
     nsteps = 4
-    f0, f, mom, _ = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=push)
+    f0, f, mom, _ = _run_partitioned(case, n_ranks, nsteps, w_fluid=0.02, push=push, own_sums=own_sums)
     st = B.DvmStepper(case)
     try:
         st.load_canonical(f0)
