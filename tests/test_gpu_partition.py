@@ -243,3 +243,47 @@ def test_fused_exchange_refuses_what_it_cannot_serve():
     finally:
         for r in ranks:
             r.close()
+
+
+def test_distributed_plumbing_of_the_fused_exchange_with_a_one_rank_nccl_group():
+    """setup_push_distributed / step_pushed_distributed with the only process group one GPU allows (world size 1, NCCL):
+    f and the carried sums in torch's symmetric memory, rendezvous, ufs_dvm_sums_use, the recv lists by all_gather_object,
+    the stream barrier.  No peer exists, so nothing crosses a wire; the result must be the plain step's, bit for bit."""
+    import os
+    import socket
+    import torch
+    import torch.distributed as dist
+    pytest.importorskip("torch.distributed._symmetric_memory")
+    from paper_1503_00707_b200.partition import exchange_distributed, setup_push_distributed, step_pushed_distributed
+    assert not dist.is_initialized()
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1")
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        case = inputs.small(3)
+        desc, keep = B.make_desc(case)
+        rol = B.ufs_dvm_partition(desc, 1)
+        r = RankStepper(case, rol, 0, 1, symmetric=True)
+        st = B.DvmStepper(case)
+        try:
+            assert B.ufs_dvm_sums_dev(r.h) == (r.sums[0].data_ptr(), r.sums[1].data_ptr())
+            assert int(r.f_symm[0].buffer_ptrs[0]) == r.f[0].data_ptr()
+            f0 = inputs.initial_f(case)
+            r.load_canonical(f0)
+            setup_push_distributed(r)
+            exchange_distributed(r)
+            for _ in range(3):
+                step_pushed_distributed(r, case.dt)
+            r.sync()
+            st.load_canonical(f0)
+            st.step(case.dt, 3)
+            st.sync()
+            assert np.array_equal(st.read_canonical(), r.read_canonical())
+        finally:
+            r.close()
+            st.close()
+    finally:
+        dist.destroy_process_group()
