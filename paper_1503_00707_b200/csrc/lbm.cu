@@ -139,8 +139,31 @@ __device__ __forceinline__ void lbm_population(const LbmParams& p, const T* __re
     if (cy != 0) my += (double)cy * acc;
     if (cz != 0) mz += (double)cz * acc;
 }
+// the same for a cell whose six upwind sources are all plain cells of the same level or coarser (one slab each): no source
+// kind to decode.  The arithmetic and its order are those of lbm_population.
+template <typename T, int Q, int I>
+__device__ __forceinline__ void lbm_population_simple(const LbmParams& p, const T* __restrict__ fin, int64_t cell, const int32_t (&src)[6],
+                                                      double dth, double (&fs)[Q], double& rho, double& mx, double& my, double& mz) {
+    constexpr int cx = lat_c(Q, I, 0), cy = lat_c(Q, I, 1), cz = lat_c(Q, I, 2);
+    constexpr int cabs = (cx < 0 ? -cx : cx) + (cy < 0 ? -cy : cy) + (cz < 0 ? -cz : cz);
+    const T* __restrict__ fi = fin + (int64_t)I * p.n_cells;
+    double acc = (double)__ldg(fi + cell) * (1.0 - dth * (double)cabs);
+    if (cx != 0) acc += dth * (double)__ldg(fi + src[cx > 0 ? 0 : 1]);
+    if (cy != 0) acc += dth * (double)__ldg(fi + src[cy > 0 ? 2 : 3]);
+    if (cz != 0) acc += dth * (double)__ldg(fi + src[cz > 0 ? 4 : 5]);
+    fs[I] = acc;
+    rho += acc;
+    if (cx != 0) mx += (double)cx * acc;
+    if (cy != 0) my += (double)cy * acc;
+    if (cz != 0) mz += (double)cz * acc;
+}
 template <typename T, int Q, int I>
 struct LbmUnroll {
+    static __device__ __forceinline__ void transport_simple(const LbmParams& p, const T* __restrict__ fin, int64_t cell, const int32_t (&src)[6],
+                                                            double dth, double (&fs)[Q], double& rho, double& mx, double& my, double& mz) {
+        lbm_population_simple<T, Q, I>(p, fin, cell, src, dth, fs, rho, mx, my, mz);
+        LbmUnroll<T, Q, I + 1>::transport_simple(p, fin, cell, src, dth, fs, rho, mx, my, mz);
+    }
     static __device__ __forceinline__ void transport(const LbmParams& p, const T* __restrict__ fin, int64_t cell, const int32_t (&src)[6],
                                                      double dth, double (&fs)[Q], double& rho, double& mx, double& my, double& mz) {
         lbm_population<T, Q, I>(p, fin, cell, src, dth, fs, rho, mx, my, mz);
@@ -162,6 +185,8 @@ struct LbmUnroll {
 };
 template <typename T, int Q>
 struct LbmUnroll<T, Q, Q> {
+    static __device__ __forceinline__ void transport_simple(const LbmParams&, const T*, int64_t, const int32_t (&)[6], double, double (&)[Q],
+                                                            double&, double&, double&, double&) {}
     static __device__ __forceinline__ void transport(const LbmParams&, const T*, int64_t, const int32_t (&)[6], double, double (&)[Q],
                                                      double&, double&, double&, double&) {}
     static __device__ __forceinline__ void relax(const LbmParams&, T*, int64_t, const double (&)[Q], double, double, double, double, double) {}
@@ -179,7 +204,9 @@ __global__ void __launch_bounds__(128, Q == 19 ? 8 : 6) k_lbm_step(const LbmPara
         const double dth = p.dt * p.inv_len * (double)(1 << r1.z);   // dt / h
         double fs[Q];
         double rho = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
-        LbmUnroll<T, Q, 0>::transport(p, fin, cell, src, dth, fs, rho, mx, my, mz);
+        // SRC_SLAB is kind 0: the six codes are then the slab numbers themselves
+        if (((r0.x | r0.y | r0.z | r0.w | r1.x | r1.y) >> SRC_SHIFT) == 0) LbmUnroll<T, Q, 0>::transport_simple(p, fin, cell, src, dth, fs, rho, mx, my, mz);
+        else LbmUnroll<T, Q, 0>::transport(p, fin, cell, src, dth, fs, rho, mx, my, mz);
         const double ux = mx / rho, uy = my / rho, uz = mz / rho;
         LbmUnroll<T, Q, 0>::relax(p, fout, cell, fs, rho, ux, uy, uz, ux * ux + uy * uy + uz * uz);
     }
