@@ -193,8 +193,16 @@ struct LbmUnroll<T, Q, Q> {
     static __device__ __forceinline__ void moments(const LbmParams&, const T*, int64_t, double&, double&, double&, double&) {}
 };
 
+// resident blocks per SM the register allocation aims at (same-box A/B of 4 / 6 / 8 for D3Q19 and 4 / 5 / 6 for D3Q27: the
+// step is latency-bound, more warps win until the spills take over)
+#ifndef LBM_MINB19
+#define LBM_MINB19 8
+#endif
+#ifndef LBM_MINB27
+#define LBM_MINB27 5
+#endif
 template <typename T, int Q>
-__global__ void __launch_bounds__(128, Q == 19 ? 8 : 6) k_lbm_step(const LbmParams p) {
+__global__ void __launch_bounds__(128, Q == 19 ? LBM_MINB19 : LBM_MINB27) k_lbm_step(const LbmParams p) {
     const T* __restrict__ fin = reinterpret_cast<const T*>(p.f_in);
     T* __restrict__ fout = reinterpret_cast<T*>(p.f_out);
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
