@@ -18,6 +18,12 @@
 // eight octants of a row block the row sums are kept as 16 sign-weighted combinations (no octant-indexed registers);
 // after the block they are expanded with the row's |xi_y|, |xi_z| to the cell's 35 velocity sums (stream_common.cuh),
 // reduced over 16 lanes by a halving butterfly and added into shared memory; the last block writes them out.
+//
+// Partitioned mesh, fused ghost exchange (PUSH instantiation; include/ufs_dvm.h: ufs_dvm_halo_push_setup; PAPER.md:185-187 does
+// this exchange as messages after the step): a thread that has formed a row of a cell some peer rank lists as a ghost cell
+// stores the same registers a second time, into that peer's ghost slab of its next f (peer memory), and the thread that
+// writes a cell's sums stores them into the peer's ghost row as well.  The flattener lists, per tile, one push entry per
+// (cell, peer); tiles with entries come first and only they are stepped by this instantiation (launch_tiles).
 #include <cmath>
 
 #include "device_util.cuh"
