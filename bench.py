@@ -10,6 +10,7 @@ SURVEY.md 8(d) row 4); both f buffers (2 x 55.8 GB) resident in HBM.  Synthetic,
     python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
     python bench.py --emulate-ranks R ...     # 1 GPU: the workload cut into R ranks with the ghost exchange
     torchrun ... bench.py --gpus N --partition  # one partitioned problem over N GPUs (NCCL ghost exchange)
+    ... --fused-exchange                      # with either of the two: the step kernel writes the peers' ghost cells itself
 
 N > 1 runs N independent replicas by default (the path is one GPU by the north star).
 """
